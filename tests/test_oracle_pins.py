@@ -199,8 +199,9 @@ def test_wgl_handles_2048_ops_64_procs_and_refutes_a_swap():
 
 def test_wgl_detects_lost_item_as_empty_violation():
     # an item enqueued and completed, then a later sequential dequeue says EMPTY
-    rows, left = gen_history(11, 8, 200, 64, p_enq=0.7)
+    rows, left = gen_history(11, 3, 40, 64, p_enq=0.7)
     t_end = max(r[6] for r in rows) + 10
+    assert left
     if left:
         rows.append((0, D, 0, ST_EMPTY, 0, t_end, t_end + 1))
         assert oracle.wgl(H(rows), 64)[0] == LIN_VIOLATION
