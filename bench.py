@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py — the paper's balanced fixed-duration micro-benchmark on B200.
+
+One "step" = one pass of the whole hot path over one batch of work: queue_reset, then ONE
+persistent fully co-resident launch of the balanced kernel (every thread loops
+enqueue(unique v); dequeue()) for warmup_ms + duration_ms, on BASELINE.json configs[1]:
+G-LFQ, capacity 2^16 uint32 payloads, thread count = full co-residency.
+
+value   = successful enqueues + successful dequeues inside the measurement windows of the K
+          timed steps / (K * t_meas)            [Mops/s; eq. (1)-(2), L350-357]
+e2e     = the same work through the C ABI with HOST buffers: per step queue_reset +
+          run_balanced (config struct in, result struct out) + queue_drain into a host
+          array; all successful ops of the launch / host wall time of those calls.
+roofline: this path has no contraction and its rings are L2-resident, so the bound is the
+          L2 atomic unit, not HBM or tensor: peak = 2 * C1, C1 = the bare warp-batched FAA
+          loop on one counter at the same occupancy, measured in this run (DESIGN.md
+          "roofline").  The algorithmic-bytes view against the measured HBM copy peak is
+          given beside it.
+cpu_baseline: the oracle's std::mutex + std::deque queue through the same loop on the host.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--kind lfq|wfq|ymc]
+N > 1: replicas only (a linearizable queue is one shared object):
+every rank runs the same workload on its own GPU, no data-path collective, scaling "weak".
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CAPACITY = 1 << 16
+WARMUP_MS, DURATION_MS = 20.0, 100.0
+ALGO_BYTES_PER_OP = {"lfq": 36.5, "wfq": 37.0, "ymc": 12.0}   # SURVEY §8(d) / DESIGN.md
+KINDS = {"lfq": 0, "wfq": 1, "ymc": 2}
+
+
+def env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------ reference arm
+def run_reference(args, rank, world):
+    """Tier rule: the reference arm is the oracle, as it stands, on the host cores."""
+    if rank != 0:
+        return
+    import oracle
+    cores = oracle.hw_threads()
+    for _ in range(args.warmup):
+        oracle.mutex_bench("balanced", cores, CAPACITY, warmup_ms=5, duration_ms=20)
+    ops = 0
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = oracle.mutex_bench("balanced", cores, CAPACITY, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS)
+        ops += r["succ_enq"] + r["succ_deq"]
+    wall = time.perf_counter() - t0
+    mops = ops / (args.steps * DURATION_MS * 1e-3) / 1e6
+    sample = f"{args.steps} x (20 ms warmup + 100 ms window), {cores} host threads, capacity 2^16"
+    line = {"impl": "reference", "metric": "queue Mops/s (balanced)", "value": mops, "unit": "Mops/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": wall / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": "BJ#2 balanced, capacity 2^16, std::mutex+std::deque on host threads", "threads": cores},
+            "cpu_baseline": {"value": mops, "unit": "Mops/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": mops, "unit": "Mops/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args, rank, world, local_rank):
+    import numpy as np
+    import torch
+    import paper_2606_01693_b200 as gq
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    kind = KINDS[args.kind]
+    full = gq.queue_max_coresident_threads(kind, 256)
+    threads = args.threads or full
+    q = gq.queue_create(kind, CAPACITY)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    run_kw = dict(threads=threads, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        flush.fill_(1)                       # L2 flushed between iterations (timing rules)
+        gq.queue_reset(q)
+        return gq.run_balanced(q, **run_kw)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    t0 = time.perf_counter()
+    results = [step() for _ in range(args.steps)]
+    barrier()
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop() if sampler else None
+
+    ops_window = sum(r["succ_enq"] + r["succ_deq"] for r in results)
+    ops_all = sum(r["tot_enq"] + r["tot_deq"] for r in results)
+    kernel_ms = sum(r["kernel_ms"] for r in results) / len(results)
+    meas_s = sum(r["meas_seconds"] for r in results)
+
+    # ---- e2e through the C ABI with host buffers (reset + run + drain to host)
+    e2e_ops, e2e_drained = 0, 0
+    barrier()
+    t1 = time.perf_counter()
+    for _ in range(args.steps):
+        gq.queue_reset(q)
+        r = gq.run_balanced(q, **run_kw)
+        left = gq.queue_drain(q, CAPACITY + 1)
+        assert r["tot_enq"] - r["tot_deq"] == len(left), "conservation violated"
+        e2e_ops += r["tot_enq"] + r["tot_deq"]
+        e2e_drained += len(left)
+    barrier()
+    e2e_wall = time.perf_counter() - t1
+
+    # ---- aggregate over ranks (replicas): ops sum, time max
+    agg = torch.tensor([ops_window, ops_all, e2e_ops], dtype=torch.float64, device="cuda")
+    tmax = torch.tensor([wall, e2e_wall, kernel_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(agg, op=dist.ReduceOp.SUM)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ops_window_all, ops_all_all, e2e_ops_all = agg.tolist()
+    wall_max, e2e_wall_max, kernel_ms_max = tmax.tolist()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        gq.queue_destroy(q)
+        return
+
+    value = ops_window_all / (args.steps * DURATION_MS * 1e-3) / 1e6
+
+    # ---- ceilings at the same occupancy (rank 0, outside the timed region)
+    c1 = gq.run_faa_ceiling(1, threads=threads, warmup_ms=5, duration_ms=30)
+    c4 = gq.run_faa_ceiling(4, threads=threads, warmup_ms=5, duration_ms=30)
+    c1_tps = c1["succ_enq"] / c1["meas_seconds"]
+    c4_tps = c4["succ_enq"] / c4["meas_seconds"]
+    peaks, peak_src = measured_peaks()
+    ops_per_s_kernel = (ops_all / len(results)) / (kernel_ms * 1e-3)      # whole launch / event duration
+    algo_gbps = ops_per_s_kernel * ALGO_BYTES_PER_OP[args.kind] / 1e9
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.kind)
+    except Exception:
+        pass
+    roofline = {"bound": "l2_atomic", "achieved": ops_per_s_kernel / 1e9, "peak": 2 * c1_tps / 1e9, "unit": "Gop/s",
+                "frac": ops_per_s_kernel / (2 * c1_tps), "traffic": traffic,
+                "kernel": "gqk::bench_kernel", "kernel_ms": kernel_ms,
+                "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run",
+                "c1_gtickets_s": c1_tps / 1e9, "c4_gtickets_s": c4_tps / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),
+                "algorithmic_GBps": algo_gbps, "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src,
+                "hbm_frac": algo_gbps / peaks["hbm_gbs"]}
+
+    # ---- thread sweep of BJ#2 and the producer-fraction sweep of BJ#3 (context, not timed)
+    sweep = {}
+    if not args.no_sweep:
+        for name, k in KINDS.items():
+            try:
+                fk = gq.queue_max_coresident_threads(k, 256)
+                qq = gq.queue_create(k, CAPACITY)
+            except gq.GqError:
+                continue
+            pts = {}
+            for th in (32, 256, 2048, 16384, 65536, fk):
+                gq.queue_reset(qq)
+                r = gq.run_balanced(qq, threads=th, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns)
+                pts[str(th)] = round(r["mops"], 1)
+            gq.queue_destroy(qq)
+            sweep["balanced_" + name] = pts
+            try:
+                qq = gq.queue_create(k, 1 << 20)
+                pre = np.arange(1 << 19, dtype=np.uint32)
+                pts = {}
+                for pf in (0.1, 0.25, 0.5, 0.75, 0.9):
+                    gq.queue_reset(qq)
+                    gq.queue_prefill(qq, pre)
+                    r = gq.run_split(qq, threads=fk, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=pf,
+                                     seed=1, value_base=1 << 19, fail_backoff_ns=args.fail_backoff_ns)
+                    pts[str(pf)] = {"enq_mops": round(r["succ_enq"] / r["meas_seconds"] / 1e6, 1),
+                                    "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1),
+                                    "full_rate": round(r["full"] / max(1, r["full"] + r["succ_enq"]), 4),
+                                    "empty_rate": round(r["empty"] / max(1, r["empty"] + r["succ_deq"]), 4)}
+                gq.queue_destroy(qq)
+                sweep["split_" + name] = pts
+            except gq.GqError as e:
+                sweep["split_" + name] = str(e)
+
+    # ---- CPU baseline: the oracle, as it stands, on this box's host cores (bounded sample)
+    import oracle
+    cores = oracle.hw_threads()
+    best = None
+    tcount = 1
+    cand = []
+    while tcount < cores:
+        cand.append(tcount); tcount *= 2
+    cand.append(cores)
+    for t in cand:
+        rs = [oracle.mutex_bench("balanced", t, CAPACITY, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS)["mops"] for _ in range(3)]
+        m = statistics.median(rs)
+        if best is None or m > best[0]:
+            best = (m, t)
+    cpu_baseline = {"value": best[0], "unit": "Mops/s", "cores": best[1], "kind": "oracle", "host_cores": cores,
+                    "sample": f"std::mutex+std::deque, balanced loop, capacity 2^16, 20+100 ms x 3 (median) at threads {cand}; best shown"}
+
+    line = {
+        "metric": "queue Mops/s (balanced)", "value": value, "unit": "Mops/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": wall_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": f"BJ#2 balanced fixed-duration: {args.kind} capacity 2^16 uint32, {threads} threads "
+                               f"(full co-residency = {full}), block 256, 20 ms warmup + 100 ms window per step",
+                   "kind": args.kind, "threads": threads, "capacity": CAPACITY, "fail_backoff_ns": args.fail_backoff_ns,
+                   "l2": "256 MiB device buffer written between steps (L2 flush); rings are L2-resident by design",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "e2e": {"value": e2e_ops_all / e2e_wall_max / 1e6, "unit": "Mops/s", "h2d_bytes_per_step": 64,
+                "d2h_bytes_per_step": 128 + 8 + 4 * (e2e_drained // args.steps),
+                "what": "queue_reset + run_balanced + queue_drain(host array) per step; all successful ops of the launch / host wall time"},
+        "gpu_launches": args.steps * 3,      # per step: 2 format kernels (queue_reset) + 1 bench kernel
+        "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline, "sweep": sweep,
+        "conservation": "checked every e2e step: tot_enq - tot_deq == drained",
+    }
+    print(json.dumps(line), flush=True)
+    gq.queue_destroy(q)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kind", default="lfq", choices=list(KINDS))
+    ap.add_argument("--threads", type=int, default=0, help="0 = full co-residency")
+    ap.add_argument("--fail-backoff-ns", type=int, default=0)
+    ap.add_argument("--no-sweep", action="store_true")
+    args = ap.parse_args()
+    rank, world, local_rank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,152 @@
+/* gq.h — C ABI of the B200-native concurrent-queue library (libgq.so).
+ *
+ * Implements the three linearizable bounded GPU queues of "Scalable Concurrent Queues for
+ * GPU" (arxiv 2606.01693; cited below as P:Lnnn = reference/PAPER.md line nnn):
+ *   GQ_LFQ      G-LFQ      lock-free sCQ-style ring, warp-batched FAA     P:L86-228  §III-B, Alg. 1
+ *   GQ_WFQ      G-WFQ      + bounded wait-free slow path, 64-bit CAS only P:L230-331 §III-C, Alg. 2
+ *   GQ_WFQ_YMC  G-WFQ-YMC  Yang/Mellor-Crummey queue on a preallocated pool P:L80-84 §III-A
+ *
+ * The queue operation itself (enqueue / dequeue issued by every resident thread) is a
+ * __device__ API: include/gq/queue.cuh.  This header is the host boundary: plain pointers
+ * and sizes, no C++ or torch types.  Every step runs in the library's own CUDA kernels;
+ * there is no CPU fallback: without a CUDA device every compute entry point returns
+ * GQ_E_CUDA.
+ *
+ * Conventions
+ *  - Every function returns int: 0 = success, negative = error (below).  Out-parameters are
+ *    written only on success (run_* also fill *res on GQ_E_POOL with the partial counters).
+ *  - "host" / "device" is stated for every pointer.  Streams are cudaStream_t passed as
+ *    void* (NULL = default stream).  Calls are synchronous on that stream.
+ *  - Ownership: queue_create allocates device memory owned by the handle until
+ *    queue_destroy.  With gq_opts.storage the caller (e.g. torch) owns the device block and
+ *    the library only formats it.  Caller buffers stay the caller's.
+ *  - A handle is not safe for concurrent host calls.
+ */
+#ifndef GQ_H_
+#define GQ_H_
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { GQ_LFQ = 0, GQ_WFQ = 1, GQ_WFQ_YMC = 2 };             /* kind */
+enum { GQ_OK = 0, GQ_FULL = 1, GQ_EMPTY = 2 };               /* device-op status */
+enum { GQ_E_INVAL = -1, GQ_E_NOMEM = -2, GQ_E_CUDA = -3, GQ_E_RESIDENCY = -4,
+       GQ_E_TIMEOUT = -5, GQ_E_STATE = -6, GQ_E_POOL = -7 };
+enum { GQ_OP_ENQ = 0, GQ_OP_DEQ = 1 };                       /* op=0 ENQ, op=1 DEQ */
+
+#define GQ_PATIENCE_ZERO 0xFFFFFFFFu   /* patience value meaning "no fast attempts": every op takes the slow path */
+
+typedef struct gq_queue gq_queue;      /* opaque host handle */
+
+/* All fields 0 = default. */
+typedef struct {
+  uint32_t max_threads;     /* k upper bound: sizes per-thread records and the ring parameter
+                               N = max(capacity, pow2ceil(max_threads)) (reading G1);
+                               default = full co-residency of the benchmark kernel */
+  uint32_t enq_patience;    /* G-WFQ / YMC fast attempts before the slow path; default 16 / 10 */
+  uint32_t deq_patience;    /* default 64 / 10 */
+  uint32_t help_delay;      /* D: inspect one peer record every D operations; default 64 */
+  uint64_t ymc_pool_cells;  /* G-WFQ-YMC preallocated cells; default 2^26 */
+  void*    storage;         /* optional caller-owned DEVICE block of >= queue_storage_bytes() bytes, 256 B aligned */
+  size_t   storage_bytes;
+  uint32_t layout;          /* ring entry stride: 0 = dense 8 B (default), 1 = 32 B sector, 2 = 128 B line */
+  uint32_t flags;           /* GQ_F_* */
+} gq_opts;
+enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the warp-batched one ("naive") */
+       GQ_F_NO_PROBE = 2u,      /* ablation: no read-only emptiness probe before a ticket is claimed (D1) */
+       GQ_F_NO_DEQ_SPIN = 4u    /* ablation: dequeuer invalidates a vacant slot at once, no bounded wait (D2) */ };
+
+/* Device bytes queue_create_ex would need for (kind, capacity, opts). */
+size_t queue_storage_bytes(int kind, uint64_t capacity, const gq_opts* opts);
+/* Create a queue of logical capacity n = `capacity` uint32 payloads ("logical capacity n").
+   capacity >= 1.  GQ_WFQ_YMC: capacity does not throttle, the pool does (reading Y3). */
+int queue_create   (int kind, uint64_t capacity, gq_queue** out);
+int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts, gq_queue** out);
+int queue_destroy  (gq_queue* q);
+/* Back to the empty initial state (reading G4). */
+int queue_reset    (gq_queue* q, void* stream);
+/* Enqueue host_vals[0..count) in array order (one warp, so FIFO order = array order).
+   Returns GQ_E_STATE if fewer than `count` fit.  host_vals: HOST. */
+int queue_prefill  (gq_queue* q, const uint32_t* host_vals, uint64_t count, void* stream);
+/* Dequeue until EMPTY or `max` items, in FIFO order, into host_out (HOST). */
+int queue_drain    (gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream);
+/* Copy the POD device view (gq::LfqView / WfqView / YmcView of include/gq/queue.cuh) that user
+   kernels take by value.  view_out: HOST, view_bytes must be >= sizeof(view). */
+int queue_device_view(const gq_queue* q, void* view_out, size_t view_bytes);
+int queue_kind(const gq_queue* q);
+/* Largest thread count the benchmark kernel of this kind can keep co-resident (occupancy
+   API x SM count): the forward-progress assumption of Thm III.10. */
+int queue_max_coresident_threads(int kind, int block_threads, uint32_t* out);
+
+typedef struct {
+  uint32_t threads;            /* participating threads k (<= max co-resident; 0 = full co-residency) */
+  uint32_t block_threads;      /* 0 = 256 */
+  double   warmup_ms;          /* P:L359 "warmup interval followed by a measurement interval" */
+  double   duration_ms;        /* t_meas of P:L355 */
+  double   producer_fraction;  /* run_split: P(thread is a producer) */
+  uint64_t seed;               /* roles, jitter */
+  uint32_t record_history;     /* 1: log {proc,op,arg,ret,call,end} per op; needs ops_per_thread > 0 */
+  uint32_t ops_per_thread;     /* > 0: fixed-op mode (iterations per thread) instead of fixed duration */
+  uint32_t jitter_ns;          /* random __nanosleep in [0, jitter_ns] before each op (history runs) */
+  uint32_t fail_backoff_ns;    /* harness sleeps up to this long after a FULL/EMPTY return (0 = none) */
+  uint64_t value_base;         /* first payload value (split: prefill size) */
+} gq_run_cfg;
+
+typedef struct {
+  uint64_t succ_enq, succ_deq, full, empty;      /* inside the measurement window */
+  uint64_t tot_enq, tot_deq, tot_full, tot_empty;/* whole kernel, for conservation */
+  uint64_t sum_enq, sum_deq;                     /* sums of OK payloads, mod 2^64, whole kernel */
+  uint64_t slow_enq, slow_deq, helps, retries;   /* G-WFQ / YMC slow-path entries, helps given, ring retries */
+  double   meas_seconds;                         /* t_meas (fixed-op mode: kernel device time) */
+  double   kernel_ms;                            /* CUDA-event time of the benchmark kernel */
+  uint32_t threads_launched, blocks, blocks_per_sm, pool_exhausted;
+} gq_run_result;
+
+/* P:L349 balanced kernel: every thread loops { enqueue(unique v); dequeue() }.  The queue is
+   NOT reset first.  Fixed-op mode runs cfg->ops_per_thread iterations per thread. */
+int run_balanced(gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res);
+/* P:L349 split kernel: thread is a pure producer iff mix32(seed, tid) < producer_fraction * 2^32. */
+int run_split   (gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res);
+/* Ceiling C1: bare warp-batched FAA (Alg. 1 WAVEFAA) on one counter, nothing else.
+   res->succ_enq = tickets taken inside the window.  n_counters in {1,4}: 4 = each warp cycles
+   over four padded counters (the like-for-like ceiling for one enqueue+dequeue pair). */
+int run_faa_ceiling(const gq_run_cfg* cfg, uint32_t n_counters, gq_run_result* res);
+/* Ceiling C2: coalesced stream of 64-bit CAS + red.or over a ring-sized L2-resident buffer. */
+int run_slot_atomic_ceiling(const gq_run_cfg* cfg, uint64_t slots, gq_run_result* res);
+
+/* Lemma III.1 probe: `threads` threads call the warp-batched FAA `rounds` times inside
+   seeded divergent control flow; tickets_out (HOST, threads*rounds entries, UINT64_MAX = lane did
+   not participate that round); *final_counter = counter value at the end. */
+int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint64_t* tickets_out, uint64_t* final_counter);
+
+/* Single-thread script: op[i] in {GQ_OP_ENQ, GQ_OP_DEQ}, arg[i] payload; results to HOST arrays.
+   `tid` = the thread_ctx id used (exercises per-thread records). */
+int queue_run_script(gq_queue* q, const uint32_t* host_op, const uint32_t* host_arg, uint64_t count,
+                     uint32_t tid, uint32_t* host_status, uint32_t* host_val);
+
+typedef struct { uint32_t proc, op, arg, ret_status, ret_val, _pad; uint64_t call_ns, end_ns; } gq_hist_rec;
+/* Records of the last record_history run, thread-major.  host_out: HOST. */
+int history_dump(gq_queue* q, gq_hist_rec* host_out, uint64_t max, uint64_t* n_out);
+
+/* Level-synchronous BFS with two alternating frontier queues.  d_rowptr (nv+1 uint64),
+   d_col (uint32), d_dist (nv int32, output; -1 = unreachable): DEVICE.  stats_out: HOST gq_bfs_stats. */
+typedef struct { uint32_t levels; uint32_t threads; uint64_t edges_scanned, vertices_visited, queue_ops; double ms; } gq_bfs_stats;
+int bfs_run(int kind, const uint64_t* d_rowptr, const uint32_t* d_col, uint32_t nv, uint32_t src,
+            int32_t* d_dist, gq_bfs_stats* stats_out, void* stream);
+
+/* Tile-based persistent wavefront tracer with a work queue of tile ids (BASELINE.json config 5). */
+typedef struct { uint32_t width, height, spp, max_bounce, n_spheres, threads; uint64_t seed;
+                 const float* d_spheres; /* DEVICE, n_spheres x 8: cx,cy,cz,r, ar,ag,ab, emissive(0/1) */ } gq_rt_scene;
+typedef struct { uint64_t rays, queue_ops; double ms; } gq_rt_stats;
+int rt_render(int kind, const gq_rt_scene* scene, float* d_rgb /* DEVICE H*W*3 */, gq_rt_stats* stats_out, void* stream);
+
+const char* gq_last_cuda_error(void);   /* text of the last CUDA error seen by this thread */
+const char* gq_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GQ_H_ */

@@ -1,0 +1,153 @@
+// gq/detail/prim.cuh — device primitives for sm_100a.
+//
+// Memory-model wrappers.  Every shared word of the queues is accessed through these: explicit
+// order (.relaxed / .acquire / .release), explicit scope (.gpu) and explicit state space
+// (.global).  They are what cuda::atomic_ref<T, thread_scope_device> means, minus its
+// generic-address lowering: on sm_100a nvcc 12.9 turns atomic_ref on a generic pointer into
+// ATOM.E + an ATOMS.CAST.SPIN shared-memory fallback branch per call and never emits RED for
+// a discarded result.  With .global the SASS is one
+// ATOMG / REDG / LDG.STRONG.GPU per call.
+//
+// WAVEFAA (Alg. 1, Lemma III.1) is warp_faa() below, re-derived for
+// 32-lane warps with independent thread scheduling (reading G10).
+#pragma once
+#include <cstdint>
+
+namespace gq {
+namespace detail {
+
+__device__ __forceinline__ uint32_t lane_id() { uint32_t l; asm("mov.u32 %0, %%laneid;" : "=r"(l)); return l; }
+__device__ __forceinline__ uint32_t lanemask_lt() { uint32_t m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
+// %globaltimer: ns, one clock for the whole GPU.  volatile + memory clobber keep the read
+// where it is written relative to the surrounding memory operations (reading H1).
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+  uint64_t t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory"); return t;
+}
+
+// ---- loads / stores -------------------------------------------------------------------
+__device__ __forceinline__ uint64_t ld_relaxed(const uint64_t* p) {
+  uint64_t v; asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ uint64_t ld_acquire(const uint64_t* p) {
+  uint64_t v; asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ uint32_t ld_relaxed32(const uint32_t* p) {
+  uint32_t v; asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ uint32_t ld_acquire32(const uint32_t* p) {
+  uint32_t v; asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ void st_relaxed(uint64_t* p, uint64_t v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void st_release(uint64_t* p, uint64_t v) {
+  asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void st_relaxed32(uint32_t* p, uint32_t v) {
+  asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void st_release32(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void fence_acq_rel() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+
+// ---- read-modify-write ----------------------------------------------------------------
+__device__ __forceinline__ uint64_t faa_relaxed(uint64_t* p, uint64_t v) {
+  uint64_t o; asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(o) : "l"(p), "l"(v) : "memory"); return o;
+}
+__device__ __forceinline__ void red_add_relaxed(uint64_t* p, uint64_t v) {
+  asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void red_or_relaxed(uint64_t* p, uint64_t v) {
+  asm volatile("red.relaxed.gpu.global.or.b64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ uint64_t fetch_max_relaxed(uint64_t* p, uint64_t v) {
+  uint64_t o; asm volatile("atom.relaxed.gpu.global.max.u64 %0, [%1], %2;" : "=l"(o) : "l"(p), "l"(v) : "memory"); return o;
+}
+__device__ __forceinline__ void red_max_relaxed(uint64_t* p, uint64_t v) {
+  asm volatile("red.relaxed.gpu.global.max.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+// CAS returning the value found (success iff result == expected).
+__device__ __forceinline__ uint64_t cas_relaxed(uint64_t* p, uint64_t expected, uint64_t desired) {
+  uint64_t o; asm volatile("atom.relaxed.gpu.global.cas.b64 %0, [%1], %2, %3;" : "=l"(o) : "l"(p), "l"(expected), "l"(desired) : "memory"); return o;
+}
+__device__ __forceinline__ uint64_t cas_release(uint64_t* p, uint64_t expected, uint64_t desired) {
+  uint64_t o; asm volatile("atom.release.gpu.global.cas.b64 %0, [%1], %2, %3;" : "=l"(o) : "l"(p), "l"(expected), "l"(desired) : "memory"); return o;
+}
+__device__ __forceinline__ uint64_t cas_acq_rel(uint64_t* p, uint64_t expected, uint64_t desired) {
+  uint64_t o; asm volatile("atom.acq_rel.gpu.global.cas.b64 %0, [%1], %2, %3;" : "=l"(o) : "l"(p), "l"(expected), "l"(desired) : "memory"); return o;
+}
+__device__ __forceinline__ uint32_t cas_relaxed32(uint32_t* p, uint32_t expected, uint32_t desired) {
+  uint32_t o; asm volatile("atom.relaxed.gpu.global.cas.b32 %0, [%1], %2, %3;" : "=r"(o) : "l"(p), "r"(expected), "r"(desired) : "memory"); return o;
+}
+__device__ __forceinline__ uint32_t cas_acq_rel32(uint32_t* p, uint32_t expected, uint32_t desired) {
+  uint32_t o; asm volatile("atom.acq_rel.gpu.global.cas.b32 %0, [%1], %2, %3;" : "=r"(o) : "l"(p), "r"(expected), "r"(desired) : "memory"); return o;
+}
+
+// ---- WAVEFAA --------------------------------------------------------------------------
+// PAPER.md Alg. 1: mask <- Ballot(active); count <- Popcount(mask); leader <-
+// FirstSetBit(mask)-1; leader: base <- FAA(C, count); base <- Shuffle(base, leader);
+// rank <- Popcount(mask & lower_lanes(lane)); return base + rank.
+//
+// sm_100a: the "active" set is whatever group of lanes is converged here.  kUniform = true
+// takes __activemask() as is (all converged callers name the same counter: benchmark
+// kernels, where divergence by role already splits the groups).  kUniform = false groups
+// lanes by counter address with match.any first, so converged lanes may target different
+// queues.  The one mask is used for leader, rank and shuffle; lanes outside it take no part,
+// and no lane waits for a lane outside its own mask (reading G10).  `unit` scales the add
+// for packed counters (G-WFQ: unit = 1 << THRIDX_BITS); the returned value is the raw word
+// base + rank*unit.
+template <bool kUniform>
+__device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 1) {
+  uint32_t mask = __activemask();
+  if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
+  const uint32_t leader = __ffs(mask) - 1;
+  const uint32_t rank = __popc(mask & lanemask_lt());
+  uint64_t base = 0;
+  if (lane_id() == leader) base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);
+  base = __shfl_sync(mask, base, leader);
+  return base + (uint64_t)rank * unit;
+}
+// The "naive" per-thread FAA of PAPER.md L95, kept for the ablation (GQ_F_PER_LANE_FAA).
+__device__ __forceinline__ uint64_t lane_faa(uint64_t* counter, uint64_t unit = 1) { return faa_relaxed(counter, unit); }
+
+// Same batching for FAA(Threshold, -1) (Alg. 1): lanes of one group get the values
+// a lane-ordered sequence of single decrements would have returned.
+template <bool kUniform>
+__device__ __forceinline__ int64_t warp_dec(int64_t* counter) {
+  uint32_t mask = __activemask();
+  if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
+  const uint32_t leader = __ffs(mask) - 1;
+  const uint32_t rank = __popc(mask & lanemask_lt());
+  uint64_t base = 0;
+  if (lane_id() == leader) base = faa_relaxed(reinterpret_cast<uint64_t*>(counter), (uint64_t)(-(int64_t)__popc(mask)));
+  base = __shfl_sync(mask, base, leader);
+  return (int64_t)base - (int64_t)rank;
+}
+
+// ---- modular cycle compare (PAPER.md Lemma III.6) -----------------------------
+// a is newer than b iff 0 < (a - b) mod R < R/2, R = 2^bits.
+template <int kBits>
+__device__ __host__ __forceinline__ bool cycle_newer(uint32_t a, uint32_t b) {
+  constexpr uint32_t R_MASK = kBits == 32 ? 0xFFFFFFFFu : ((1u << (kBits & 31)) - 1u);
+  const uint32_t d = (a - b) & R_MASK;
+  return d != 0 && d < (1u << (kBits - 1));
+}
+
+// bounded exponential backoff for retry loops (north_star: "bounded spin with __nanosleep backoff")
+struct Backoff {
+  uint32_t ns = 0;
+  __device__ __forceinline__ void pause() {
+    if (ns) __nanosleep(ns);
+    ns = ns ? (ns < 1024 ? ns * 2 : 1024) : 32;
+  }
+};
+
+// counter-based 32-bit mixer (roles, jitter): not part of any queue algorithm
+__device__ __host__ __forceinline__ uint32_t mix32(uint32_t x) {
+  x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+  return x;
+}
+
+}  // namespace detail
+}  // namespace gq

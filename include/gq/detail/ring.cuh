@@ -1,0 +1,230 @@
+// gq/detail/ring.cuh — the bounded inner ring of G-LFQ and of G-WFQ's fast path.
+//
+// PAPER.md §III-B (L88-89): "a ring of size 2n, a threshold check for empty ... Each slot is
+// a single 64-bit word ... monotonically increasing Head and Tail counters, a Threshold used
+// by empty dequeues, and the entry array itself."  Algorithm 1 (L143-211): TRYENQ, TRYDEQ.
+// SLOT(t) = t mod 2N, CYCLE(t) = floor(t / 2N) mod 2^bc (L107).  The ring is sized by
+// N = max(n, pow2ceil(k)) so that k <= N holds for any thread count (reading G1).
+//
+// sm_100a layout (reading G13): entries are dense 8-byte words with no cache remap, so the
+// 32 consecutive tickets of one warp_faa batch touch 256 contiguous bytes (8 sectors, 2 lines)
+// and are served by one coalesced L2 request per instruction; Head, Tail and Threshold each
+// sit on their own 1 KiB-strided line so that the three hot words never share an L2 slice
+// queue.  `slot_shift` spreads entries over 32 B / 128 B for the padding ablation.
+#pragma once
+#include "prim.cuh"
+
+namespace gq {
+
+struct RingView {
+  uint64_t* entry;      // 2N slots, stride 8 << slot_shift bytes
+  uint64_t* head;       // packed per format (counter << kCtrShift | ThrIdx)
+  uint64_t* tail;
+  int64_t*  threshold;  // signed; reset value 3N-1
+  uint64_t* owner;      // G-WFQ only: Owner[2N] side table (reading W6); else nullptr
+  int64_t   thr_reset;  // 3N-1
+  uint32_t  order;      // log2(2N)
+  uint32_t  slot_shift; // 0 dense, 2 = 32 B, 4 = 128 B
+};
+
+namespace detail {
+
+enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
+// GQ_F_* bits of gq.h that reach the device (kept numerically identical)
+enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u };
+
+// ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
+struct LfqFmt {
+  static constexpr int kCycBits = 31;
+  static constexpr int kCtrShift = 0;                    // Head/Tail are plain counters
+  static constexpr uint32_t kBotC = 0xFFFFFFFFu;         // consumed   (reading G3)
+  static constexpr uint32_t kBot = 0xFFFFFFFEu;          // empty
+  static constexpr uint64_t kIdxMask = 0xFFFFFFFFull;
+  static constexpr uint64_t kSafeBit = 1ull << 32;
+  static constexpr uint64_t kConsumeMask = kIdxMask;     // CONSUME = atomic OR of the index field
+  static constexpr uint32_t kCycMask = 0x7FFFFFFFu;
+  __device__ __host__ static uint32_t cycle(uint64_t e) { return (uint32_t)(e >> 33); }
+  __device__ __host__ static uint32_t index(uint64_t e) { return (uint32_t)e; }
+  __device__ __host__ static bool safe(uint64_t e) { return (e & kSafeBit) != 0; }
+  __device__ __host__ static bool enq_visible(uint64_t) { return true; }
+  __device__ __host__ static bool vacant(uint64_t e) { return index(e) >= kBot; }    // Index in {bot, botc}
+  // <c, 1, x>
+  __device__ __host__ static uint64_t installed(uint64_t, uint32_t c, uint32_t x) { return ((uint64_t)c << 33) | kSafeBit | x; }
+  // <c, E.Safe, bot>
+  __device__ __host__ static uint64_t advanced(uint64_t e, uint32_t c) { return ((uint64_t)c << 33) | (e & kSafeBit) | kBot; }
+  // <E.Cycle, 0, E.Index>
+  __device__ __host__ static uint64_t unsafe(uint64_t e) { return e & ~kSafeBit; }
+  __device__ __host__ static uint64_t initial() { return kSafeBit | kBot; }          // <0,1,bot> (reading G4)
+};
+
+// ---- G-WFQ entry word (Fig. 2 missing -> reading W1):
+//      [63:48] Cycle(16) | [47:32] Note(16) | [31] Safe | [30] Enq | [29:0] Index(30)
+struct WfqFmt {
+  static constexpr int kCycBits = 16;
+  static constexpr int kCtrShift = 20;                   // Head/Tail word: counter(44) | ThrIdx(20)
+  static constexpr uint32_t kBotC = 0x3FFFFFFFu;
+  static constexpr uint32_t kBot = 0x3FFFFFFEu;
+  static constexpr uint64_t kIdxMask = 0x3FFFFFFFull;
+  static constexpr uint64_t kEnqBit = 1ull << 30;
+  static constexpr uint64_t kSafeBit = 1ull << 31;
+  static constexpr uint64_t kNoteMask = 0xFFFFull << 32;
+  static constexpr uint64_t kConsumeMask = kIdxMask | kEnqBit;   // sets Enq=1 and Index=botc together
+  static constexpr uint32_t kCycMask = 0xFFFFu;
+  static constexpr uint64_t kThrIdxMask = (1ull << kCtrShift) - 1;
+  static constexpr uint64_t kThrNull = kThrIdxMask;
+  __device__ __host__ static uint32_t cycle(uint64_t e) { return (uint32_t)(e >> 48); }
+  __device__ __host__ static uint32_t note(uint64_t e) { return (uint32_t)(e >> 32) & 0xFFFFu; }
+  __device__ __host__ static uint32_t index(uint64_t e) { return (uint32_t)(e & kIdxMask); }
+  __device__ __host__ static bool safe(uint64_t e) { return (e & kSafeBit) != 0; }
+  __device__ __host__ static bool enq_visible(uint64_t e) { return (e & kEnqBit) != 0; }
+  __device__ __host__ static bool vacant(uint64_t e) { return index(e) >= kBot; }
+  // fast path installs <c, Safe 1, Enq 1, x>, Note unchanged
+  __device__ __host__ static uint64_t installed(uint64_t e, uint32_t c, uint32_t x) {
+    return ((uint64_t)c << 48) | (e & kNoteMask) | kSafeBit | kEnqBit | x;
+  }
+  __device__ __host__ static uint64_t installed_slow(uint64_t e, uint32_t c, uint32_t x) {   // Enq = 0
+    return ((uint64_t)c << 48) | (e & kNoteMask) | kSafeBit | x;
+  }
+  __device__ __host__ static uint64_t advanced(uint64_t e, uint32_t c) {
+    return ((uint64_t)c << 48) | (e & kNoteMask) | (e & kSafeBit) | kEnqBit | kBot;
+  }
+  __device__ __host__ static uint64_t unsafe(uint64_t e) { return e & ~kSafeBit; }
+  __device__ __host__ static uint64_t with_note(uint64_t e, uint32_t c) { return (e & ~kNoteMask) | ((uint64_t)c << 32); }
+  // Note starts "older than every cycle in use": tickets start at cycle 1, so 0 with modular compare
+  __device__ __host__ static uint64_t initial() { return kSafeBit | kEnqBit | kBot; }
+};
+
+// Hook run by a dequeuer between finding its entry and CONSUME.  G-LFQ: nothing.
+struct NoFinalize {
+  __device__ __forceinline__ void operator()(const RingView&, uint64_t /*h*/, uint32_t /*j*/, uint64_t /*E*/) const {}
+};
+
+template <class F, bool kUniform, bool kWarpFaa = true>
+struct Ring {
+  __device__ __forceinline__ static uint64_t* slot(const RingView& r, uint32_t j) {
+    return r.entry + ((size_t)j << r.slot_shift);
+  }
+  __device__ __forceinline__ static uint32_t slot_of(const RingView& r, uint64_t t) { return (uint32_t)t & ((1u << r.order) - 1u); }
+  __device__ __forceinline__ static uint32_t cycle_of(const RingView& r, uint64_t t) { return (uint32_t)(t >> r.order) & F::kCycMask; }
+  __device__ __forceinline__ static uint64_t counter(uint64_t word) { return word >> F::kCtrShift; }
+
+  // ticket reservation: WAVEFAA on a (possibly packed) counter word
+  __device__ __forceinline__ static uint64_t take(uint64_t* ctr) {
+    constexpr uint64_t unit = 1ull << F::kCtrShift;
+    const uint64_t w = kWarpFaa ? warp_faa<kUniform>(ctr, unit) : lane_faa(ctr, unit);
+    return counter(w);
+  }
+
+  // "reset Threshold to 3n-1" (Alg. 1): load first, store only when different, so the
+  // line stays clean in steady state (reading G8).
+  __device__ __forceinline__ static void reset_threshold(const RingView& r) {
+    if ((int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)) != r.thr_reset)
+      st_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)r.thr_reset);
+  }
+
+  // "catch up Tail to at least h+1" (Alg. 1; reading G9).  Batched like WAVEFAA: the
+  // converged lanes agree on their largest target and only the leader touches the hot word
+  // (one atomic per warp instead of 32 on the same address).
+  __device__ __forceinline__ static void catchup_tail(const RingView& r, uint64_t target) {
+    uint32_t mask = __activemask();
+    if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(r.tail));
+    const uint32_t leader = __ffs(mask) - 1;
+    const uint64_t base = __shfl_sync(mask, target, leader);
+    const int dmax = __reduce_max_sync(mask, (int)(int64_t)(target - base));   // tickets of one warp are close
+    if (lane_id() != leader) return;
+    target = base + (int64_t)dmax;
+    if (F::kCtrShift == 0) {
+      red_max_relaxed(r.tail, target);
+    } else {
+      uint64_t w = ld_relaxed(r.tail);
+      for (int i = 0; i < 64 && counter(w) < target; ++i) {      // bounded; counter field only grows
+        const uint64_t nw = (target << F::kCtrShift) | (w & ((1ull << F::kCtrShift) - 1));
+        const uint64_t o = cas_relaxed(r.tail, w, nw);
+        if (o == w) break;
+        w = o;
+      }
+    }
+  }
+
+  // Alg. 1 L143-163.  Returns RING_OK or RING_RETRY; *t_out = the ticket used.
+  __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out) {
+    const uint64_t t = take(r.tail);                                  // L144
+    *t_out = t;
+    const uint32_t j = slot_of(r, t), c = cycle_of(r, t);             // L146
+    uint64_t* sp = slot(r, j);
+    const uint64_t E = ld_relaxed(sp);                                // L148
+    if (cycle_newer<F::kCycBits>(c, F::cycle(E)) && F::vacant(E)) {   // E.Cycle < c, Index in {bot,botc}
+      bool ok = F::safe(E);
+      if (!ok) {                                                      // (E.Safe or Head <= t), reading G5
+        fence_acq_rel();                                              // Head must not be older than E
+        ok = counter(ld_relaxed(r.head)) <= t;
+      }
+      if (ok && cas_release(sp, E, F::installed(E, c, x)) == E) {     // L153: linearization point (L111)
+        reset_threshold(r);                                           // L155
+        return RING_OK;
+      }
+    }
+    return RING_RETRY;                                                   // L163 (reading G7)
+  }
+
+  // Alg. 1 L165-211 with the reconstruction of reading G6 (reload on CAS failure).
+  // Returns RING_OK (+ *x), RING_EMPTY or RING_RETRY; *h_out = the ticket used.
+  //
+  // Two bounded additions for sm_100a, where k >> n threads can poll an empty ring
+  // (D1, D2; each can be switched off for the ablation):
+  //  D1 read-only emptiness probe.  `probe` is set by callers whose previous attempt on this
+  //     ring came back EMPTY, and also taken when Threshold is below its reset value (some
+  //     dequeuer failed since the last successful enqueue).  Head is read first (acquire),
+  //     then Tail: Tail(t2) <= Head(t1) <= Head(t2) is the very condition of L197 ("Tail <= h+1"
+  //     seen by the owner of ticket h), observed without claiming a ticket, so an empty ring
+  //     is left undisturbed: Head does not run ahead and no slot is invalidated.
+  //  D2 bounded wait for the matching enqueuer.  A dequeuer that finds its slot still vacant
+  //     although Tail > h (an enqueuer owns ticket h and is between its FAA and its CAS)
+  //     reloads up to kDeqSpin times with __nanosleep before it invalidates the slot as
+  //     L186-188 prescribe.  Pure delay in front of the paper's steps; lock-freedom is kept.
+  static constexpr int kDeqSpin = 6;
+  template <class Finalize>
+  __device__ __forceinline__ static int try_deq(const RingView& r, uint32_t* x, uint64_t* h_out, const Finalize& fin,
+                                                bool probe = false, uint32_t flags = 0) {
+    const int64_t thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
+    if (thr < 0) return RING_EMPTY;                                   // L166-169
+    if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {       // D1
+      const uint64_t H = counter(ld_acquire(r.head));
+      if (counter(ld_relaxed(r.tail)) <= H) return RING_EMPTY;
+    }
+    const uint64_t h = take(r.head);                                  // L172
+    *h_out = h;
+    const uint32_t j = slot_of(r, h), c = cycle_of(r, h);             // L175
+    uint64_t* sp = slot(r, j);
+    int spin = (flags & kNoDeqSpin) ? 0 : kDeqSpin;
+    for (;;) {
+      const uint64_t E = ld_acquire(sp);                              // L176 (acquire: payload edge, G15)
+      if (F::cycle(E) == c && !F::vacant(E)) {                        // L178
+        fin(r, h, j, E);                                              // G-WFQ: finalize an Enq=0 entry (W6)
+        red_or_relaxed(sp, F::kConsumeMask);                          // L180 CONSUME: linearization point
+        *x = F::index(E);
+        return RING_OK;                                               // L182
+      }
+      if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
+        if (spin > 0 && F::vacant(E) && counter(ld_relaxed(r.tail)) > h) {   // D2
+          --spin; __nanosleep(64); continue;
+        }
+        const uint64_t New = F::vacant(E) ? F::advanced(E, c)         // L186-188
+                                          : F::unsafe(E);             // L193
+        if (New != E && cas_relaxed(sp, E, New) != E) continue;       // reload: the slot changed under us
+      }
+      break;
+    }
+    const uint64_t T = counter(ld_relaxed(r.tail));
+    if (T <= h + 1) {                                                 // L197
+      catchup_tail(r, h + 1);                                         // L200
+      warp_dec<kUniform>(r.threshold);                                // L202
+      return RING_EMPTY;
+    }
+    if (warp_dec<kUniform>(r.threshold) <= 0) return RING_EMPTY;      // L205-208
+    return RING_RETRY;                                                // L211
+  }
+};
+
+}  // namespace detail
+}  // namespace gq

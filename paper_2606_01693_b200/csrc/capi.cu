@@ -1,0 +1,532 @@
+// capi.cu — host side of libgq.so: handle management, memory layout in HBM, kernel launches.
+// Every entry point is declared and documented in include/gq.h.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <thread>
+#include <vector>
+
+#include "gq.h"
+#include "kernels.cuh"
+
+using namespace gq;
+using namespace gq::detail;
+using namespace gqk;
+
+// ------------------------------------------------------------------------------- errors
+static thread_local char g_err[256] = "";
+static int cuda_fail(cudaError_t e, const char* what) {
+  std::snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
+  return e == cudaErrorMemoryAllocation ? GQ_E_NOMEM : GQ_E_CUDA;
+}
+#define CU(call)                                          \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
+  } while (0)
+
+extern "C" const char* gq_last_cuda_error(void) { return g_err; }
+extern "C" const char* gq_version(void) { return "gq 0.1 (sm_100a)"; }
+
+static_assert(sizeof(gq_opts) == 48 && sizeof(gq_run_cfg) == 64 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
+              "ABI structs: the Python binding mirrors these layouts");
+
+// ------------------------------------------------------------------------------- handle
+struct gq_queue {
+  int kind = 0;
+  uint64_t capacity = 0;   // n
+  uint64_t N = 0;          // ring parameter (reading G1)
+  gq_opts opts{};
+  uint32_t max_threads = 0;
+  char* base = nullptr;    // device block
+  size_t bytes = 0;
+  bool owns = false;
+  LfqView lfq{};
+  WfqView wfq{};
+  YmcView ymc{};
+  uint64_t* d_ctr = nullptr;        // C_COUNT result counters
+  gq_hist_rec* d_hist = nullptr;
+  uint64_t hist_cap = 0, hist_n = 0;
+};
+
+static int g_sms = 0;
+static int device_sms() {
+  if (!g_sms) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
+  }
+  return g_sms;
+}
+static uint64_t pow2ceil(uint64_t x) { uint64_t p = 1; while (p < x) p <<= 1; return p; }
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------- layout
+// One device block per queue:
+//   [ hot words, one per 1 KiB ][ AQ entries ][ FQ entries ][ Data ][ kind-specific ... ]
+static constexpr size_t kHotStride = 1024;
+struct Layout {
+  uint64_t N = 0;
+  uint32_t order = 0, slot_shift = 0;
+  size_t off_hot = 0, off_aq = 0, off_fq = 0, off_data = 0, off_owner_aq = 0, off_owner_fq = 0, off_rec = 0, off_pool = 0;
+  size_t total = 0;
+  uint64_t pool_cells = 0;
+};
+
+template <class Q> static int max_blocks_per_sm(int block_threads);
+
+static uint32_t default_max_threads(int kind);
+
+static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout* L, uint32_t* max_threads_out) {
+  if (kind < GQ_LFQ || kind > GQ_WFQ_YMC || capacity < 1) return GQ_E_INVAL;
+  gq_opts z{}; if (!o) o = &z;
+  if (o->layout > 2) return GQ_E_INVAL;
+  uint32_t k = o->max_threads ? o->max_threads : default_max_threads(kind);
+  if (k == 0) k = 148 * 2048;                         // no device visible: size for a full B200
+  *max_threads_out = k;
+  size_t off = 0;
+  L->off_hot = off; off += 16 * kHotStride;
+  if (kind == GQ_LFQ || kind == GQ_WFQ) {
+    const uint64_t idx_limit = kind == GQ_LFQ ? 0xFFFFFFFEull : 0x3FFFFFFEull;
+    if (capacity >= idx_limit) return GQ_E_INVAL;
+    if (kind == GQ_WFQ && k >= WfqFmt::kThrNull) return GQ_E_INVAL;
+    L->N = pow2ceil(std::max<uint64_t>(capacity, k));
+    L->order = 0; while ((1ull << L->order) < 2 * L->N) ++L->order;
+    L->slot_shift = o->layout == 0 ? 0 : (o->layout == 1 ? 2 : 4);
+    const size_t ring_bytes = (size_t)(2 * L->N) * (8u << L->slot_shift);
+    L->off_aq = off; off += ring_bytes;
+    L->off_fq = off; off += ring_bytes;
+    L->off_data = off; off += align_up((size_t)capacity * 4, 256);
+    if (kind == GQ_WFQ) {
+      L->off_owner_aq = off; off += (size_t)(2 * L->N) * 8;
+      L->off_owner_fq = off; off += (size_t)(2 * L->N) * 8;
+      L->off_rec = off; off += (size_t)k * sizeof(WfqRecord);
+    }
+  } else {
+    L->pool_cells = o->ymc_pool_cells ? o->ymc_pool_cells : (1ull << 26);
+    L->off_rec = off; off += (size_t)k * sizeof(YmcHandle);
+    L->off_pool = off; off += (size_t)L->pool_cells * sizeof(YmcCell);
+  }
+  L->total = align_up(off, 256);
+  return 0;
+}
+
+extern "C" size_t queue_storage_bytes(int kind, uint64_t capacity, const gq_opts* opts) {
+  Layout L; uint32_t k;
+  if (compute_layout(kind, capacity, opts, &L, &k) != 0) return 0;
+  return L.total;
+}
+
+// ------------------------------------------------------------------------------- format
+// Initial states (reading G4).  empty ring: Head = Tail = 2N, entries <0,1,bot>, Threshold = -1.
+// ring pre-loaded with indices 0..count-1: Tail = 2N+count, slot i<count = <1,1,i>, Threshold = 3N-1.
+template <class F>
+__global__ void format_ring_kernel(RingView r, uint64_t slots, uint64_t count) {
+  const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < slots) {
+    uint64_t* sp = r.entry + ((size_t)i << r.slot_shift);
+    *sp = i < count ? F::installed(F::initial(), 1u, (uint32_t)i) : F::initial();
+    if (r.owner) r.owner[i] = 0;
+  }
+  if (i == 0) {
+    const uint64_t low = F::kCtrShift ? ((1ull << F::kCtrShift) - 1) : 0;   // ThrIdx = NULL
+    *r.head = (slots << F::kCtrShift) | low;
+    *r.tail = ((slots + count) << F::kCtrShift) | low;
+    *r.threshold = count ? r.thr_reset : -1;
+  }
+}
+
+static RingView make_ring(char* base, const Layout& L, size_t off_entries, size_t off_owner, int hot_slot) {
+  RingView r{};
+  r.entry = reinterpret_cast<uint64_t*>(base + off_entries);
+  r.head = reinterpret_cast<uint64_t*>(base + L.off_hot + (hot_slot + 0) * kHotStride);
+  r.tail = reinterpret_cast<uint64_t*>(base + L.off_hot + (hot_slot + 1) * kHotStride);
+  r.threshold = reinterpret_cast<int64_t*>(base + L.off_hot + (hot_slot + 2) * kHotStride);
+  r.owner = off_owner ? reinterpret_cast<uint64_t*>(base + off_owner) : nullptr;
+  r.thr_reset = (int64_t)(3 * L.N - 1);
+  r.order = L.order;
+  r.slot_shift = L.slot_shift;
+  return r;
+}
+
+static int format_queue(gq_queue* q, cudaStream_t st) {
+  const uint64_t slots = 2 * q->N;
+  const unsigned blk = 256, grd = (unsigned)((slots + blk - 1) / blk);
+  if (q->kind == GQ_LFQ) {
+    format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.aq, slots, 0);
+    format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.fq, slots, q->capacity);
+  } else {
+    return GQ_E_INVAL;
+  }
+  CU(cudaGetLastError());
+  return 0;
+}
+
+// ------------------------------------------------------------------------------- occupancy
+template <class Q>
+static int max_blocks_per_sm(int block_threads) {
+  int nb = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, bench_kernel<Q, false, true>, block_threads, 0) != cudaSuccess) return 0;
+  return nb;
+}
+static int kind_blocks_per_sm(int kind, int block_threads) {
+  switch (kind) {
+    case GQ_LFQ: return max_blocks_per_sm<LfqView>(block_threads);
+    default: return 0;
+  }
+}
+static uint32_t default_max_threads(int kind) {
+  const int sms = device_sms();
+  if (sms <= 0) return 0;
+  return (uint32_t)(kind_blocks_per_sm(kind, 256) * 256 * sms);
+}
+
+extern "C" int queue_max_coresident_threads(int kind, int block_threads, uint32_t* out) {
+  if (!out || kind < GQ_LFQ || kind > GQ_WFQ_YMC) return GQ_E_INVAL;
+  if (block_threads <= 0) block_threads = 256;
+  if (block_threads % 32 || block_threads > 512) return GQ_E_INVAL;
+  const int sms = device_sms();
+  if (sms <= 0) { std::snprintf(g_err, sizeof g_err, "no CUDA device"); return GQ_E_CUDA; }
+  const int nb = kind_blocks_per_sm(kind, block_threads);
+  if (nb <= 0) return GQ_E_CUDA;
+  *out = (uint32_t)(nb * block_threads * sms);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------- create / destroy
+extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts, gq_queue** out) {
+  if (!out) return GQ_E_INVAL;
+  if (device_sms() <= 0) { std::snprintf(g_err, sizeof g_err, "no CUDA device"); return GQ_E_CUDA; }
+  Layout L; uint32_t k = 0;
+  int rc = compute_layout(kind, capacity, opts, &L, &k);
+  if (rc) return rc;
+  gq_queue* q = new (std::nothrow) gq_queue();
+  if (!q) return GQ_E_NOMEM;
+  q->kind = kind; q->capacity = capacity; q->N = L.N; q->max_threads = k;
+  if (opts) q->opts = *opts;
+  q->bytes = L.total;
+  if (opts && opts->storage) {
+    if (opts->storage_bytes < L.total || (reinterpret_cast<uintptr_t>(opts->storage) & 255)) { delete q; return GQ_E_INVAL; }
+    q->base = static_cast<char*>(opts->storage);
+  } else {
+    cudaError_t e = cudaMalloc(&q->base, L.total);
+    if (e != cudaSuccess) { delete q; return cuda_fail(e, "cudaMalloc(queue)"); }
+    q->owns = true;
+  }
+  cudaError_t e = cudaMalloc(&q->d_ctr, C_COUNT * sizeof(uint64_t));
+  if (e != cudaSuccess) { if (q->owns) cudaFree(q->base); delete q; return cuda_fail(e, "cudaMalloc(counters)"); }
+  if (kind == GQ_LFQ) {
+    q->lfq.aq = make_ring(q->base, L, L.off_aq, 0, 0);
+    q->lfq.fq = make_ring(q->base, L, L.off_fq, 0, 3);
+    q->lfq.data = reinterpret_cast<uint32_t*>(q->base + L.off_data);
+    q->lfq.capacity = (uint32_t)capacity;
+    q->lfq.flags = q->opts.flags;
+  }
+  rc = format_queue(q, nullptr);
+  if (rc == 0) { cudaError_t e2 = cudaDeviceSynchronize(); if (e2 != cudaSuccess) rc = cuda_fail(e2, "format"); }
+  if (rc) { queue_destroy(q); return rc; }
+  *out = q;
+  return 0;
+}
+extern "C" int queue_create(int kind, uint64_t capacity, gq_queue** out) { return queue_create_ex(kind, capacity, nullptr, out); }
+
+extern "C" int queue_destroy(gq_queue* q) {
+  if (!q) return GQ_E_INVAL;
+  if (q->owns && q->base) cudaFree(q->base);
+  if (q->d_ctr) cudaFree(q->d_ctr);
+  if (q->d_hist) cudaFree(q->d_hist);
+  delete q;
+  return 0;
+}
+
+extern "C" int queue_reset(gq_queue* q, void* stream) {
+  if (!q) return GQ_E_INVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int rc = format_queue(q, st);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(st));
+  return 0;
+}
+
+extern "C" int queue_kind(const gq_queue* q) { return q ? q->kind : GQ_E_INVAL; }
+
+extern "C" int queue_device_view(const gq_queue* q, void* view_out, size_t view_bytes) {
+  if (!q || !view_out) return GQ_E_INVAL;
+  const void* src = nullptr; size_t n = 0;
+  switch (q->kind) {
+    case GQ_LFQ: src = &q->lfq; n = sizeof(LfqView); break;
+    case GQ_WFQ: src = &q->wfq; n = sizeof(WfqView); break;
+    default: src = &q->ymc; n = sizeof(YmcView); break;
+  }
+  if (view_bytes < n) return GQ_E_INVAL;
+  std::memcpy(view_out, src, n);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------- launches
+// Wait for `ev` with a host-side watchdog so that a livelocked kernel fails a call instead of
+// hanging it (SURVEY §5 "failure detection").
+static int wait_event(cudaEvent_t ev, double budget_s) {
+  const auto t0 = std::chrono::steady_clock::now();
+  for (;;) {
+    cudaError_t e = cudaEventQuery(ev);
+    if (e == cudaSuccess) return 0;
+    if (e != cudaErrorNotReady) return cuda_fail(e, "kernel");
+    if (std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count() > budget_s) {
+      std::snprintf(g_err, sizeof g_err, "watchdog: kernel still running after %.0f s", budget_s);
+      return GQ_E_TIMEOUT;
+    }
+    std::this_thread::sleep_for(std::chrono::microseconds(200));
+  }
+}
+
+struct Resolved { uint32_t threads, block, blocks, blocks_per_sm; };
+static int resolve_launch(int blocks_per_sm, const gq_run_cfg* cfg, uint32_t thread_cap, Resolved* r) {
+  const int sms = device_sms();
+  if (sms <= 0) { std::snprintf(g_err, sizeof g_err, "no CUDA device"); return GQ_E_CUDA; }
+  r->block = cfg->block_threads ? cfg->block_threads : 256;
+  if (r->block % 32 || r->block > 512) return GQ_E_INVAL;
+  if (blocks_per_sm <= 0) return GQ_E_CUDA;
+  const uint32_t full = (uint32_t)blocks_per_sm * r->block * sms;
+  r->threads = cfg->threads ? cfg->threads : std::min(full, thread_cap);
+  if (r->threads > thread_cap) return GQ_E_INVAL;
+  r->blocks = (r->threads + r->block - 1) / r->block;
+  r->blocks_per_sm = (uint32_t)blocks_per_sm;
+  if (r->blocks > (uint32_t)blocks_per_sm * sms) return GQ_E_RESIDENCY;   // Thm III.10 assumption
+  return 0;
+}
+
+static BenchParams make_params(const gq_run_cfg* cfg, const Resolved& r, int mode) {
+  BenchParams p{};
+  p.threads = r.threads; p.mode = (uint32_t)mode;
+  p.warmup_ns = (uint64_t)(cfg->warmup_ms * 1e6); p.duration_ns = (uint64_t)(cfg->duration_ms * 1e6);
+  double pf = cfg->producer_fraction; if (pf < 0) pf = 0; if (pf > 1) pf = 1;
+  p.prod_threshold = (uint64_t)(pf * 4294967296.0);
+  p.seed = (uint32_t)cfg->seed; p.ops_per_thread = cfg->ops_per_thread;
+  p.jitter_ns = cfg->jitter_ns; p.fail_backoff_ns = cfg->fail_backoff_ns; p.value_base = cfg->value_base;
+  return p;
+}
+
+static int finish_run(uint64_t* d_ctr, cudaEvent_t e0, cudaEvent_t e1, const gq_run_cfg* cfg, const Resolved& r, gq_run_result* res) {
+  uint64_t c[C_COUNT];
+  CU(cudaMemcpy(c, d_ctr, sizeof c, cudaMemcpyDeviceToHost));
+  float ms = 0; CU(cudaEventElapsedTime(&ms, e0, e1));
+  std::memset(res, 0, sizeof *res);
+  res->succ_enq = c[C_SUCC_ENQ]; res->succ_deq = c[C_SUCC_DEQ]; res->full = c[C_FULL]; res->empty = c[C_EMPTY];
+  res->tot_enq = c[C_TOT_ENQ]; res->tot_deq = c[C_TOT_DEQ]; res->tot_full = c[C_TOT_FULL]; res->tot_empty = c[C_TOT_EMPTY];
+  res->sum_enq = c[C_SUM_ENQ]; res->sum_deq = c[C_SUM_DEQ]; res->retries = c[C_RETRIES];
+  res->kernel_ms = ms;
+  res->meas_seconds = cfg->ops_per_thread ? (double)(c[C_T_END] - c[C_T0]) * 1e-9 : cfg->duration_ms * 1e-3;
+  res->threads_launched = r.threads; res->blocks = r.blocks; res->blocks_per_sm = r.blocks_per_sm;
+  res->pool_exhausted = (uint32_t)(c[C_POOL] != 0);
+  return 0;
+}
+
+template <class Q>
+static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mode, gq_run_result* res) {
+  const bool per_lane = (q->opts.flags & GQ_F_PER_LANE_FAA) != 0;
+  const bool hist = cfg->record_history != 0;
+  if (hist && cfg->ops_per_thread == 0) return GQ_E_INVAL;
+  if (!hist && cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
+  void* fn = hist ? (per_lane ? (void*)bench_kernel<Q, true, false> : (void*)bench_kernel<Q, true, true>)
+                  : (per_lane ? (void*)bench_kernel<Q, false, false> : (void*)bench_kernel<Q, false, true>);
+  Resolved r;
+  int nb = 0;
+  const uint32_t blk = cfg->block_threads ? cfg->block_threads : 256;
+  if (blk % 32 || blk > 512) return GQ_E_INVAL;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, (int)blk, 0));
+  int rc = resolve_launch(nb, cfg, q->max_threads, &r);
+  if (rc) return rc;
+  if (hist) {
+    const uint64_t need = (uint64_t)r.threads * cfg->ops_per_thread * (mode == MODE_SPLIT ? 1 : 2);
+    if (need > q->hist_cap) {
+      if (q->d_hist) cudaFree(q->d_hist);
+      q->d_hist = nullptr; q->hist_cap = 0;
+      CU(cudaMalloc(&q->d_hist, need * sizeof(gq_hist_rec)));
+      q->hist_cap = need;
+    }
+    q->hist_n = need;
+  }
+  CU(cudaMemset(q->d_ctr, 0, C_COUNT * sizeof(uint64_t)));
+  BenchParams p = make_params(cfg, r, mode);
+  Q v = view;
+  uint64_t* ctr = q->d_ctr; gq_hist_rec* h = q->d_hist;
+  void* args[] = {&v, &p, &ctr, &h};
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  CU(cudaEventRecord(e0, nullptr));
+  cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
+  if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return le == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : cuda_fail(le, "launch"); }
+  CU(cudaEventRecord(e1, nullptr));
+  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + 60.0);
+  if (rc == 0) rc = finish_run(q->d_ctr, e0, e1, cfg, r, res);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (rc == 0 && res->pool_exhausted) return GQ_E_POOL;
+  return rc;
+}
+
+static int run_bench(gq_queue* q, const gq_run_cfg* cfg, int mode, gq_run_result* res) {
+  if (!q || !cfg || !res) return GQ_E_INVAL;
+  switch (q->kind) {
+    case GQ_LFQ: return run_bench_t<LfqView>(q, q->lfq, cfg, mode, res);
+    default: return GQ_E_INVAL;
+  }
+}
+extern "C" int run_balanced(gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res) { return run_bench(q, cfg, MODE_BALANCED, res); }
+extern "C" int run_split(gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res) { return run_bench(q, cfg, MODE_SPLIT, res); }
+
+// ------------------------------------------------------------------------------- ceilings
+template <class K, class... A>
+static int run_ceiling(K kernel, const gq_run_cfg* cfg, gq_run_result* res, uint64_t* d_ctr, void** args) {
+  int nb = 0;
+  const uint32_t blk = cfg->block_threads ? cfg->block_threads : 256;
+  if (blk % 32 || blk > 512) return GQ_E_INVAL;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, (int)blk, 0));
+  Resolved r;
+  int rc = resolve_launch(nb, cfg, 0xFFFFFFFFu, &r);
+  if (rc) return rc;
+  BenchParams p = make_params(cfg, r, MODE_BALANCED);
+  args[2] = &p;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  CU(cudaEventRecord(e0, nullptr));
+  cudaError_t le = cudaLaunchCooperativeKernel((void*)kernel, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
+  if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return cuda_fail(le, "launch"); }
+  CU(cudaEventRecord(e1, nullptr));
+  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + 60.0);
+  if (rc == 0) rc = finish_run(d_ctr, e0, e1, cfg, r, res);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return rc;
+}
+
+extern "C" int run_faa_ceiling(const gq_run_cfg* cfg, uint32_t n_counters, gq_run_result* res) {
+  if (!cfg || !res || n_counters < 1 || n_counters > 8) return GQ_E_INVAL;
+  if (cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
+  uint64_t *d_counters = nullptr, *d_ctr = nullptr;
+  CU(cudaMalloc(&d_counters, 8 * 1024));
+  cudaError_t e = cudaMalloc(&d_ctr, C_COUNT * 8);
+  if (e != cudaSuccess) { cudaFree(d_counters); return cuda_fail(e, "cudaMalloc"); }
+  cudaMemset(d_counters, 0, 8 * 1024); cudaMemset(d_ctr, 0, C_COUNT * 8);
+  void* args[4] = {&d_counters, &n_counters, nullptr, &d_ctr};
+  int rc = run_ceiling(faa_ceiling_kernel<true>, cfg, res, d_ctr, args);
+  cudaFree(d_counters); cudaFree(d_ctr);
+  return rc;
+}
+
+extern "C" int run_slot_atomic_ceiling(const gq_run_cfg* cfg, uint64_t slots, gq_run_result* res) {
+  if (!cfg || !res || slots < 32) return GQ_E_INVAL;
+  if (cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
+  uint64_t *d_buf = nullptr, *d_ctr = nullptr;
+  CU(cudaMalloc(&d_buf, slots * 8));
+  cudaError_t e = cudaMalloc(&d_ctr, C_COUNT * 8);
+  if (e != cudaSuccess) { cudaFree(d_buf); return cuda_fail(e, "cudaMalloc"); }
+  cudaMemset(d_buf, 0, slots * 8); cudaMemset(d_ctr, 0, C_COUNT * 8);
+  void* args[4] = {&d_buf, &slots, nullptr, &d_ctr};
+  int rc = run_ceiling(slot_ceiling_kernel, cfg, res, d_ctr, args);
+  cudaFree(d_buf); cudaFree(d_ctr);
+  return rc;
+}
+
+extern "C" int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint64_t* tickets_out, uint64_t* final_counter) {
+  if (!threads || !rounds || !tickets_out || !final_counter) return GQ_E_INVAL;
+  if (device_sms() <= 0) { std::snprintf(g_err, sizeof g_err, "no CUDA device"); return GQ_E_CUDA; }
+  uint64_t *d_c = nullptr, *d_t = nullptr;
+  const size_t n = (size_t)threads * rounds;
+  CU(cudaMalloc(&d_c, 8));
+  cudaError_t e = cudaMalloc(&d_t, n * 8);
+  if (e != cudaSuccess) { cudaFree(d_c); return cuda_fail(e, "cudaMalloc"); }
+  cudaMemset(d_c, 0, 8);
+  warp_faa_probe_kernel<<<(threads + 255) / 256, 256>>>(d_c, threads, rounds, (uint32_t)seed, d_t);
+  e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaMemcpy(tickets_out, d_t, n * 8, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(final_counter, d_c, 8, cudaMemcpyDeviceToHost);
+  cudaFree(d_c); cudaFree(d_t);
+  return e == cudaSuccess ? 0 : cuda_fail(e, "warp_faa_probe");
+}
+
+// ------------------------------------------------------------------------------- prefill / drain / script / history
+template <class Q>
+static int prefill_t(const Q& view, const uint32_t* host_vals, uint64_t count, cudaStream_t st) {
+  uint32_t* d_vals = nullptr; uint64_t* d_n = nullptr;
+  CU(cudaMalloc(&d_vals, std::max<uint64_t>(count, 1) * 4));
+  cudaError_t e = cudaMalloc(&d_n, 8);
+  if (e != cudaSuccess) { cudaFree(d_vals); return cuda_fail(e, "cudaMalloc"); }
+  uint64_t n_ok = 0;
+  e = cudaMemcpyAsync(d_vals, host_vals, count * 4, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) { prefill_kernel<Q><<<1, 32, 0, st>>>(view, d_vals, count, d_n); e = cudaGetLastError(); }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&n_ok, d_n, 8, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_vals); cudaFree(d_n);
+  if (e != cudaSuccess) return cuda_fail(e, "prefill");
+  return n_ok == count ? 0 : GQ_E_STATE;
+}
+extern "C" int queue_prefill(gq_queue* q, const uint32_t* host_vals, uint64_t count, void* stream) {
+  if (!q || (!host_vals && count)) return GQ_E_INVAL;
+  if (count == 0) return 0;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  switch (q->kind) {
+    case GQ_LFQ: return prefill_t<LfqView>(q->lfq, host_vals, count, st);
+    default: return GQ_E_INVAL;
+  }
+}
+
+template <class Q>
+static int drain_t(const Q& view, uint32_t* host_out, uint64_t max, uint64_t* n_out, cudaStream_t st) {
+  uint32_t* d_out = nullptr; uint64_t* d_n = nullptr;
+  CU(cudaMalloc(&d_out, std::max<uint64_t>(max, 1) * 4));
+  cudaError_t e = cudaMalloc(&d_n, 8);
+  if (e != cudaSuccess) { cudaFree(d_out); return cuda_fail(e, "cudaMalloc"); }
+  uint64_t n = 0;
+  drain_kernel<Q><<<1, 32, 0, st>>>(view, d_out, max, d_n);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&n, d_n, 8, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess && n) e = cudaMemcpy(host_out, d_out, n * 4, cudaMemcpyDeviceToHost);
+  cudaFree(d_out); cudaFree(d_n);
+  if (e != cudaSuccess) return cuda_fail(e, "drain");
+  *n_out = n;
+  return 0;
+}
+extern "C" int queue_drain(gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream) {
+  if (!q || !n_out || (!host_out && max)) return GQ_E_INVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  switch (q->kind) {
+    case GQ_LFQ: return drain_t<LfqView>(q->lfq, host_out, max, n_out, st);
+    default: return GQ_E_INVAL;
+  }
+}
+
+template <class Q>
+static int script_t(const Q& view, const uint32_t* op, const uint32_t* arg, uint64_t count, uint32_t tid, uint32_t* st_out, uint32_t* val_out) {
+  uint32_t* d = nullptr;
+  CU(cudaMalloc(&d, count * 16));
+  uint32_t *d_op = d, *d_arg = d + count, *d_st = d + 2 * count, *d_val = d + 3 * count;
+  cudaError_t e = cudaMemcpy(d_op, op, count * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d_arg, arg, count * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) { script_kernel<Q><<<1, 1>>>(view, d_op, d_arg, count, tid, d_st, d_val); e = cudaDeviceSynchronize(); }
+  if (e == cudaSuccess) e = cudaMemcpy(st_out, d_st, count * 4, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(val_out, d_val, count * 4, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  return e == cudaSuccess ? 0 : cuda_fail(e, "script");
+}
+extern "C" int queue_run_script(gq_queue* q, const uint32_t* host_op, const uint32_t* host_arg, uint64_t count,
+                                uint32_t tid, uint32_t* host_status, uint32_t* host_val) {
+  if (!q || !host_op || !host_arg || !host_status || !host_val || tid >= q->max_threads) return GQ_E_INVAL;
+  if (count == 0) return 0;
+  switch (q->kind) {
+    case GQ_LFQ: return script_t<LfqView>(q->lfq, host_op, host_arg, count, tid, host_status, host_val);
+    default: return GQ_E_INVAL;
+  }
+}
+
+extern "C" int history_dump(gq_queue* q, gq_hist_rec* host_out, uint64_t max, uint64_t* n_out) {
+  if (!q || !n_out || (!host_out && max)) return GQ_E_INVAL;
+  const uint64_t n = std::min(max, q->hist_n);
+  if (n) CU(cudaMemcpy(host_out, q->d_hist, n * sizeof(gq_hist_rec), cudaMemcpyDeviceToHost));
+  *n_out = n;
+  return 0;
+}

@@ -1,0 +1,235 @@
+// Harness kernels: the paper's balanced / split micro-benchmarks as one
+// persistent, fully co-resident kernel (Thm III.10 residency assumption, L327-331), the
+// device-side history recorder (L335), and the small service kernels behind the C ABI.
+#pragma once
+#include <cooperative_groups.h>
+#include <cstdint>
+
+#include "gq.h"
+#include "gq/queue.cuh"
+
+namespace gqk {
+namespace cg = cooperative_groups;
+using namespace gq;
+using namespace gq::detail;
+
+enum { MODE_BALANCED = 0, MODE_SPLIT = 1 };
+// counter slots in the device result block
+enum { C_SUCC_ENQ, C_SUCC_DEQ, C_FULL, C_EMPTY, C_TOT_ENQ, C_TOT_DEQ, C_TOT_FULL, C_TOT_EMPTY,
+       C_SUM_ENQ, C_SUM_DEQ, C_RETRIES, C_T0, C_T_END, C_POOL, C_COUNT = 16 };
+
+struct BenchParams {
+  uint32_t threads, mode;
+  uint64_t warmup_ns, duration_ns;
+  uint64_t prod_threshold;     // producer iff mix32(..) < prod_threshold  (p * 2^32)
+  uint32_t seed, ops_per_thread;
+  uint32_t jitter_ns, fail_backoff_ns;
+  uint64_t value_base;
+};
+
+__device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
+#pragma unroll
+  for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// One kernel for both micro-benchmarks.  kHist: record {proc,op,arg,ret,call,end} per op.
+template <class Q, bool kHist, bool kWarpFaa>
+__global__ void __launch_bounds__(512) bench_kernel(Q q, BenchParams p, uint64_t* ctr, gq_hist_rec* hist) {
+  cg::grid_group grid = cg::this_grid();
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid == 0) st_relaxed(ctr + C_T0, globaltimer_ns());
+  grid.sync();                                        // one time base for every thread
+  const uint64_t t0 = ld_relaxed(ctr + C_T0);
+  const bool fixed = p.ops_per_thread != 0;
+  const uint64_t tw = fixed ? 0 : t0 + p.warmup_ns;
+  const uint64_t te = fixed ? ~0ull : tw + p.duration_ns;
+
+  uint32_t succ_enq = 0, succ_deq = 0, full = 0, empty = 0, tot_enq = 0, tot_deq = 0, tot_full = 0, tot_empty = 0;
+  uint64_t sum_enq = 0, sum_deq = 0, retries = 0;
+
+  if (tid < p.threads) {
+    thread_ctx ctx{tid};
+    bool do_enq = true, do_deq = true;
+    if (p.mode == MODE_SPLIT) {
+      do_enq = (uint64_t)mix32(p.seed * 0x9e3779b9u + tid) < p.prod_threshold;
+      do_deq = !do_enq;
+    }
+    const uint32_t per_iter = p.mode == MODE_SPLIT ? 1 : 2;
+    gq_hist_rec* my = kHist ? hist + (size_t)tid * p.ops_per_thread * per_iter : nullptr;
+    uint32_t fail_ns = 0;
+    for (uint32_t iter = 0;; ++iter) {
+      uint64_t now = 0;
+      if (do_enq) {
+        const uint32_t v = (uint32_t)(p.value_base + tid + (uint64_t)iter * p.threads);
+        uint64_t t_call = 0;
+        if (kHist) {
+          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (tid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
+          t_call = globaltimer_ns();
+        }
+        const int s = enqueue<true, kWarpFaa>(q, ctx, v, &retries);
+        if (kHist) { __threadfence(); }               // effects performed before `end` is read (reading H1)
+        now = globaltimer_ns();
+        if (kHist) *my++ = gq_hist_rec{tid, GQ_OP_ENQ, v, (uint32_t)s, 0u, 0u, t_call, now};
+        const bool in = now >= tw && now < te;
+        if (s == OK) { ++tot_enq; sum_enq += v; succ_enq += in; fail_ns = 0; }
+        else {
+          ++tot_full; full += in;
+          if (p.fail_backoff_ns) { fail_ns = fail_ns ? min(fail_ns * 2, p.fail_backoff_ns) : 64; __nanosleep(fail_ns); }
+        }
+      }
+      if (do_deq) {
+        uint32_t v = 0;
+        uint64_t t_call = 0;
+        if (kHist) {
+          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (tid * 0xc2b2ae35u) ^ (iter * 2u + 0x7654321u)) % (p.jitter_ns + 1));
+          t_call = globaltimer_ns();
+        }
+        const int s = dequeue<true, kWarpFaa>(q, ctx, &v, &retries);
+        if (kHist) { __threadfence(); }
+        now = globaltimer_ns();
+        if (kHist) *my++ = gq_hist_rec{tid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
+        const bool in = now >= tw && now < te;
+        if (s == OK) { ++tot_deq; sum_deq += v; succ_deq += in; fail_ns = 0; }
+        else {
+          ++tot_empty; empty += in;
+          if (p.fail_backoff_ns) { fail_ns = fail_ns ? min(fail_ns * 2, p.fail_backoff_ns) : 64; __nanosleep(fail_ns); }
+        }
+      }
+      if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
+    }
+  }
+  __syncwarp();
+  // warp-reduce, one atomic per warp per counter
+  uint64_t vals[11] = {succ_enq, succ_deq, full, empty, tot_enq, tot_deq, tot_full, tot_empty, sum_enq, sum_deq, retries};
+#pragma unroll
+  for (int i = 0; i < 11; ++i) {
+    const uint64_t s = warp_sum(vals[i]);
+    if (lane_id() == 0 && s) red_add_relaxed(ctr + i, s);
+  }
+  if (tid == 0) red_max_relaxed(ctr + C_T_END, globaltimer_ns());
+}
+
+// ---- service kernels --------------------------------------------------------------------
+// One warp enqueues vals[0..count) in array order (quiescent queue: lane order = ticket order).
+template <class Q>
+__global__ void prefill_kernel(Q q, const uint32_t* vals, uint64_t count, uint64_t* n_ok) {
+  thread_ctx ctx{threadIdx.x};
+  uint64_t ok = 0;
+  for (uint64_t base = 0; base < count; base += 32) {
+    const uint64_t i = base + threadIdx.x;
+    if (i < count && enqueue<true, true>(q, ctx, vals[i]) == OK) ++ok;
+    __syncwarp();
+  }
+  ok = warp_sum(ok);
+  if (threadIdx.x == 0) *n_ok = ok;
+}
+
+// One warp dequeues until EMPTY (or max) in FIFO order.
+template <class Q>
+__global__ void drain_kernel(Q q, uint32_t* out, uint64_t max, uint64_t* n_out) {
+  thread_ctx ctx{threadIdx.x};
+  uint64_t n = 0;
+  for (;;) {
+    const uint64_t want = max - n < 32 ? max - n : 32;
+    if (want == 0) break;
+    uint32_t v = 0;
+    int s = EMPTY;
+    if (threadIdx.x < want) s = dequeue<true, true>(q, ctx, &v);
+    __syncwarp();
+    const uint32_t okmask = __ballot_sync(0xffffffffu, s == OK);
+    if (s == OK) out[n + __popc(okmask & lanemask_lt())] = v;
+    n += __popc(okmask);
+    if (__popc(okmask) < (int)want) break;
+  }
+  if (threadIdx.x == 0) *n_out = n;
+}
+
+// Single thread runs a script of operations (differential test against the sequential model).
+template <class Q>
+__global__ void script_kernel(Q q, const uint32_t* op, const uint32_t* arg, uint64_t count, uint32_t tid,
+                              uint32_t* status, uint32_t* val) {
+  thread_ctx ctx{tid};
+  for (uint64_t i = 0; i < count; ++i) {
+    uint32_t v = 0;
+    const int s = op[i] == GQ_OP_ENQ ? enqueue<false, true>(q, ctx, arg[i]) : dequeue<false, true>(q, ctx, &v);
+    status[i] = (uint32_t)s;
+    val[i] = v;
+  }
+}
+
+// Lemma III.1 probe: warp_faa inside seeded, nested divergent control flow.
+__global__ void warp_faa_probe_kernel(uint64_t* counter, uint32_t threads, uint32_t rounds, uint32_t seed, uint64_t* tickets) {
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= threads) return;
+  for (uint32_t r = 0; r < rounds; ++r) {
+    const uint32_t h = mix32(seed ^ (tid * 0x9e3779b9u) ^ (r * 0x85ebca6bu));
+    uint64_t t = ~0ull;
+    if (h & 1) {                       // participate?
+      if (h & 2) {                     // two diverged groups name the same counter
+        if (h & 4) __nanosleep(h >> 24);
+        t = warp_faa<true>(counter);
+      } else {
+        t = warp_faa<false>(counter);  // address-matched variant
+      }
+    }
+    tickets[(size_t)tid * rounds + r] = t;
+  }
+}
+
+// Ceiling C1: bare WAVEFAA loop (BASELINE.json north_star: "a bare warp-aggregated FAA loop on one
+// counter at the same occupancy").  counters are 1 KiB apart.
+template <bool kWarpFaa>
+__global__ void __launch_bounds__(512) faa_ceiling_kernel(uint64_t* counters, uint32_t n_counters, BenchParams p, uint64_t* ctr) {
+  cg::grid_group grid = cg::this_grid();
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid == 0) st_relaxed(ctr + C_T0, globaltimer_ns());
+  grid.sync();
+  const uint64_t t0 = ld_relaxed(ctr + C_T0);
+  const bool fixed = p.ops_per_thread != 0;
+  const uint64_t tw = fixed ? 0 : t0 + p.warmup_ns, te = fixed ? ~0ull : tw + p.duration_ns;
+  uint64_t n_in = 0, n_tot = 0, acc = 0;
+  if (tid < p.threads) {
+    for (uint32_t iter = 0;; ++iter) {
+      uint64_t* c = counters + (size_t)(iter % n_counters) * 128;
+      acc ^= kWarpFaa ? warp_faa<true>(c) : lane_faa(c);
+      const uint64_t now = globaltimer_ns();
+      ++n_tot; n_in += (now >= tw && now < te);
+      if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
+    }
+  }
+  __syncwarp();
+  const uint64_t a = warp_sum(n_in), b = warp_sum(n_tot), x = warp_sum(acc);
+  if (lane_id() == 0) { if (a) red_add_relaxed(ctr + C_SUCC_ENQ, a); if (b) red_add_relaxed(ctr + C_TOT_ENQ, b); if (x == 1) red_add_relaxed(ctr + C_RETRIES, 1); }
+  if (tid == 0) red_max_relaxed(ctr + C_T_END, globaltimer_ns());
+}
+
+// Ceiling C2: what one ring operation does to its slot, without tickets: a coalesced
+// {8 B load, 64-bit CAS, red.or} stream over `slots` consecutive words.
+__global__ void __launch_bounds__(512) slot_ceiling_kernel(uint64_t* buf, uint64_t slots, BenchParams p, uint64_t* ctr) {
+  cg::grid_group grid = cg::this_grid();
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid == 0) st_relaxed(ctr + C_T0, globaltimer_ns());
+  grid.sync();
+  const uint64_t t0 = ld_relaxed(ctr + C_T0);
+  const bool fixed = p.ops_per_thread != 0;
+  const uint64_t tw = fixed ? 0 : t0 + p.warmup_ns, te = fixed ? ~0ull : tw + p.duration_ns;
+  uint64_t n_in = 0, n_tot = 0;
+  if (tid < p.threads) {
+    for (uint32_t iter = 0;; ++iter) {
+      uint64_t* s = buf + ((uint64_t)tid + (uint64_t)iter * p.threads) % slots;
+      const uint64_t e = ld_relaxed(s);
+      cas_relaxed(s, e, e + 2);
+      red_or_relaxed(s, 1);
+      const uint64_t now = globaltimer_ns();
+      ++n_tot; n_in += (now >= tw && now < te);
+      if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
+    }
+  }
+  __syncwarp();
+  const uint64_t a = warp_sum(n_in), b = warp_sum(n_tot);
+  if (lane_id() == 0) { if (a) red_add_relaxed(ctr + C_SUCC_ENQ, a); if (b) red_add_relaxed(ctr + C_TOT_ENQ, b); }
+  if (tid == 0) red_max_relaxed(ctr + C_T_END, globaltimer_ns());
+}
+
+}  // namespace gqk

@@ -1,0 +1,221 @@
+"""GPU parity tests: the CUDA queues (through the C ABI) against the oracle.
+
+Several results are correct for a concurrent queue, so parity is membership: the recorded
+history must be linearizable w.r.t. the sequential bounded FIFO,
+conserve items, and keep per-producer order (L336); single-threaded runs must equal the
+sequential model exactly, EMPTY/FULL included.  All integer: bit-exact.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2606_01693_b200 as gq
+
+pytestmark = pytest.mark.gpu
+
+KINDS = [gq.GQ_LFQ]
+IDS = [gq.KIND_NAMES[k] for k in KINDS]
+
+
+def make(kind, capacity, **opts):
+    o = gq.gq_opts(**opts)
+    return gq.queue_create_ex(kind, capacity, o)
+
+
+def to_history(recs):
+    return oracle.History(recs["proc"], recs["op"], recs["arg"], recs["ret_status"], recs["ret_val"],
+                          recs["call_ns"], recs["end_ns"])
+
+
+# ---------------------------------------------------------------- a1: WAVEFAA, Lemma III.1
+@pytest.mark.parametrize("threads,rounds,seed", [(32, 8, 1), (5000, 64, 2), (65536 + 17, 16, 3)])
+def test_warp_faa_tickets_distinct_and_contiguous(threads, rounds, seed):
+    t, final = gq.run_warp_faa_probe(threads, rounds, seed)
+    took = t[t != np.uint64(0xFFFFFFFFFFFFFFFF)]
+    assert final == len(took)
+    assert np.array_equal(np.sort(took), np.arange(len(took), dtype=np.uint64))
+    assert 0.3 < len(took) / t.size < 0.7          # the seeded divergence really split the warps
+
+
+# ---------------------------------------------------------------- single thread == sequential model
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("capacity", [1, 2, 3, 128])
+def test_single_thread_equals_model(kind, capacity):
+    rng = np.random.default_rng(capacity)
+    n_ops = 6000
+    # biased phases so that both FULL and EMPTY are hit repeatedly
+    p = np.repeat(rng.choice([0.3, 0.5, 0.7], n_ops // 200), 200)
+    ops = (rng.random(n_ops) > p).astype(np.uint32)            # 0 ENQ, 1 DEQ
+    args = np.arange(1, n_ops + 1, dtype=np.uint32)
+    q = make(kind, capacity, max_threads=64)
+    try:
+        st, val = gq.queue_run_script(q, ops, args, tid=5)
+    finally:
+        gq.queue_destroy(q)
+    est, eval_ = oracle.fifo_replay(capacity, ops, args)
+    assert np.array_equal(st, est)
+    ok_deq = (ops == 1) & (est == 0)
+    assert np.array_equal(val[ok_deq], eval_[ok_deq])
+    assert (est == oracle.ST_FULL).any() and (est == oracle.ST_EMPTY).any()
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_fresh_fill_full_drain(kind):
+    n = 128
+    q = make(kind, n, max_threads=64)
+    try:
+        ops = [1] + [0] * (n + 1) + [1] * (n + 1)
+        args = [0] + list(range(1000, 1000 + n + 1)) + [0] * (n + 1)
+        st, val = gq.queue_run_script(q, ops, args)
+        assert st[0] == gq.GQ_EMPTY
+        assert (st[1:n + 1] == gq.GQ_OK).all() and st[n + 1] == gq.GQ_FULL
+        assert val[n + 2:2 * n + 2].tolist() == list(range(1000, 1000 + n)) and st[-1] == gq.GQ_EMPTY
+    finally:
+        gq.queue_destroy(q)
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("capacity,count", [(1024, 1000), (1024, 77), (1024, 1024), (100, 0), (5, 5)])
+def test_prefill_drain_preserves_order(kind, capacity, count):
+    q = make(kind, capacity, max_threads=64)
+    try:
+        vals = (np.arange(count, dtype=np.uint32) * 7 + 3)
+        gq.queue_prefill(q, vals)
+        out = gq.queue_drain(q, capacity + 10)
+        assert np.array_equal(out, vals)
+        assert len(gq.queue_drain(q, 10)) == 0
+        if count:
+            with pytest.raises(gq.GqError):            # does not fit: GQ_E_STATE
+                gq.queue_prefill(q, np.arange(capacity + 1, dtype=np.uint32))
+            gq.queue_reset(q)
+            assert len(gq.queue_drain(q, 10)) == 0
+    finally:
+        gq.queue_destroy(q)
+
+
+# ---------------------------------------------------------------- BJ config 1: tiny history
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("seed", list(range(1, 9)))
+def test_tiny_balanced_history_is_linearizable(kind, seed):
+    q = make(kind, 128, max_threads=64)
+    try:
+        r = gq.run_balanced(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
+                            jitter_ns=200, seed=seed)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, 256)
+    finally:
+        gq.queue_destroy(q)
+    assert len(recs) == 2048 and r["blocks"] == 1
+    # reading H6: neither EMPTY nor FULL can legally occur in this configuration
+    assert r["tot_full"] == 0 and r["tot_empty"] == 0 and len(left) == 0
+    enq = recs[recs["op"] == 0]
+    assert sorted(enq["arg"].tolist()) == sorted(t + i * 64 for t in range(64) for i in range(16))
+    ok, msg = oracle.check_history(to_history(recs), 128, relaxed_full=False, leftover=left)
+    assert ok, msg
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("pf,seed", [(0.25, 1), (0.25, 2), (0.75, 3), (0.75, 4), (0.5, 5)])
+def test_tiny_split_history_with_empty_and_full(kind, pf, seed):
+    # reading H6: n = 16, 64 threads, 16 ops each: EMPTY frequent at 25 % producers, FULL at 75 %
+    q = make(kind, 16, max_threads=64)
+    try:
+        r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
+                         jitter_ns=200, seed=seed, producer_fraction=pf)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, 64)
+    finally:
+        gq.queue_destroy(q)
+    assert len(recs) == 1024
+    assert len(left) <= 16
+    if pf < 0.5:
+        assert r["tot_empty"] > 0
+    if pf > 0.5:
+        assert r["tot_full"] > 0
+    ok, msg = oracle.check_history(to_history(recs), 16, relaxed_full=True, leftover=left)
+    assert ok, msg
+
+
+# ---------------------------------------------------------------- conservation at scale
+def _conserve(r, left, prefill_vals=()):
+    pre = np.asarray(prefill_vals, dtype=np.uint64)
+    assert r["tot_enq"] + len(pre) - r["tot_deq"] == len(left)
+    s_left = int(np.asarray(left, dtype=np.uint64).sum()) if len(left) else 0
+    assert (r["sum_enq"] + int(pre.sum()) - r["sum_deq"] - s_left) % 2**64 == 0
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("threads,capacity", [(2048 + 32 + 5, 1 << 12), (0, 1 << 16)])
+def test_balanced_fixed_ops_conserves(kind, threads, capacity):
+    q = gq.queue_create(kind, capacity)
+    try:
+        r = gq.run_balanced(q, threads=threads, ops_per_thread=32)
+        left = gq.queue_drain(q, capacity + 1)
+    finally:
+        gq.queue_destroy(q)
+    assert len(left) <= capacity
+    assert r["tot_enq"] + r["tot_full"] == r["threads_launched"] * 32
+    assert r["tot_deq"] + r["tot_empty"] == r["threads_launched"] * 32
+    _conserve(r, left)
+    assert len(set(left.tolist())) == len(left)
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_balanced_timed_full_occupancy(kind):
+    # BJ config 2 at full co-residency, shortened window; same launch configuration as bench.py
+    q = gq.queue_create(kind, 1 << 16)
+    try:
+        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=20)
+        left = gq.queue_drain(q, (1 << 16) + 1)
+    finally:
+        gq.queue_destroy(q)
+    assert r["threads_launched"] == gq.queue_max_coresident_threads(kind, 256)
+    assert r["succ_enq"] > 0 and r["succ_deq"] > 0
+    assert len(left) <= 1 << 16
+    _conserve(r, left)
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("pf", [0.1, 0.5, 0.9])
+def test_split_timed_conserves(kind, pf):
+    # BJ config 3 shape (capacity 2^20 prefilled to 50 %), shortened window
+    n = 1 << 20
+    pre = np.arange(n // 2, dtype=np.uint32)
+    q = gq.queue_create(kind, n)
+    try:
+        gq.queue_prefill(q, pre)
+        r = gq.run_split(q, threads=0, warmup_ms=2, duration_ms=10, producer_fraction=pf, seed=7, value_base=n // 2)
+        left = gq.queue_drain(q, n + 1)
+    finally:
+        gq.queue_destroy(q)
+    assert len(left) <= n
+    _conserve(r, left, pre)
+    # FIFO: what is left of the prefill comes out first and in order
+    pre_left = left[left < n // 2]
+    assert np.array_equal(pre_left, np.sort(pre_left)) and np.array_equal(left[: len(pre_left)], pre_left)
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_token_protocol_at_scale(kind):
+    # exactly once, no foreign token, per-producer monotone — 16384 threads
+    q = gq.queue_create(kind, 1 << 14)
+    try:
+        gq.run_split(q, threads=16384, ops_per_thread=24, record_history=1, producer_fraction=0.5, seed=11)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, (1 << 14) + 1)
+    finally:
+        gq.queue_destroy(q)
+    assert len(recs) == 16384 * 24
+    h = to_history(recs)
+    assert oracle.precheck(h) == ""
+    assert oracle.conservation(h, left) == ""
+
+
+def test_residency_is_enforced():
+    q = gq.queue_create(gq.GQ_LFQ, 1024)
+    try:
+        full = gq.queue_max_coresident_threads(gq.GQ_LFQ, 256)
+        with pytest.raises(gq.GqError):
+            gq.run_balanced(q, threads=full + 256, ops_per_thread=1)
+    finally:
+        gq.queue_destroy(q)
