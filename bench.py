@@ -279,7 +279,7 @@ def run_ours(args, rank, world, local_rank):
                    "kind": args.kind, "threads": threads, "capacity": CAPACITY, "fail_backoff_ns": args.fail_backoff_ns,
                    "l2": "256 MiB device buffer written between steps (L2 flush); rings are L2-resident by design",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
-        "e2e": {"value": e2e_ops_all / e2e_wall_max / 1e6, "unit": "Mops/s", "h2d_bytes_per_step": 64,
+        "e2e": {"value": e2e_ops_all / e2e_wall_max / 1e6, "unit": "Mops/s", "h2d_bytes_per_step": 64,   # the gq_run_cfg struct
                 "d2h_bytes_per_step": 128 + 8 + 4 * (e2e_drained // args.steps),
                 "what": "queue_reset + run_balanced + queue_drain(host array) per step; all successful ops of the launch / host wall time"},
         "gpu_launches": args.steps * 3,      # per step: 2 format kernels (queue_reset) + 1 bench kernel

@@ -54,10 +54,13 @@ typedef struct {
   size_t   storage_bytes;
   uint32_t layout;          /* ring entry stride: 0 = dense 8 B (default), 1 = 32 B sector, 2 = 128 B line */
   uint32_t flags;           /* GQ_F_* */
+  uint32_t park_ns;         /* longest wait of a dequeuer on its own vacant slot before it gives the slot up
+                               (D2); default 250000 */
+  uint32_t _reserved;
 } gq_opts;
 enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the warp-batched one ("naive") */
        GQ_F_NO_PROBE = 2u,      /* ablation: no read-only emptiness probe before a ticket is claimed (D1) */
-       GQ_F_NO_DEQ_SPIN = 4u    /* ablation: dequeuer invalidates a vacant slot at once, no bounded wait (D2) */ };
+       GQ_F_NO_DEQ_SPIN = 4u    /* ablation: dequeuer invalidates a vacant slot at once, no parking (D2) */ };
 
 /* Device bytes queue_create_ex would need for (kind, capacity, opts). */
 size_t queue_storage_bytes(int kind, uint64_t capacity, const gq_opts* opts);

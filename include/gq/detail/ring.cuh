@@ -22,9 +22,12 @@ struct RingView {
   uint64_t* tail;
   int64_t*  threshold;  // signed; reset value 3N-1
   uint64_t* owner;      // G-WFQ only: Owner[2N] side table (reading W6); else nullptr
+  void*     rec;        // G-WFQ only: WfqRecord[k] of this ring; else nullptr
   int64_t   thr_reset;  // 3N-1
   uint32_t  order;      // log2(2N)
   uint32_t  slot_shift; // 0 dense, 2 = 32 B, 4 = 128 B
+  uint32_t  park_ns;    // D2: longest time a dequeuer waits on its own vacant slot (0 = never)
+  uint32_t  park_limit; // D1: EMPTY without a ticket once Head is this far ahead of Tail
 };
 
 namespace detail {
@@ -171,32 +174,37 @@ struct Ring {
   // Returns RING_OK (+ *x), RING_EMPTY or RING_RETRY; *h_out = the ticket used.
   //
   // Two bounded additions for sm_100a, where k >> n threads can poll an empty ring
-  // (D1, D2; each can be switched off for the ablation):
-  //  D1 read-only emptiness probe.  `probe` is set by callers whose previous attempt on this
-  //     ring came back EMPTY, and also taken when Threshold is below its reset value (some
-  //     dequeuer failed since the last successful enqueue).  Head is read first (acquire),
-  //     then Tail: Tail(t2) <= Head(t1) <= Head(t2) is the very condition of L197 ("Tail <= h+1"
-  //     seen by the owner of ticket h), observed without claiming a ticket, so an empty ring
-  //     is left undisturbed: Head does not run ahead and no slot is invalidated.
-  //  D2 bounded wait for the matching enqueuer.  A dequeuer that finds its slot still vacant
-  //     although Tail > h (an enqueuer owns ticket h and is between its FAA and its CAS)
-  //     reloads up to kDeqSpin times with __nanosleep before it invalidates the slot as
-  //     L186-188 prescribe.  Pure delay in front of the paper's steps; lock-freedom is kept.
-  static constexpr int kDeqSpin = 6;
+  // (DESIGN.md "departures" D1, D2; each can be switched off for the ablation):
+  //  D1 read-only emptiness probe.  Taken when the caller's previous attempt on this ring came
+  //     back EMPTY (`probe`) or Threshold is below its reset value (some dequeuer failed since
+  //     the last successful enqueue).  Head is read first (acquire), then Tail:
+  //     Tail(t2) <= Head(t1) <= Head(t2) is the very condition of L197 ("Tail <= h+1" seen by
+  //     the owner of ticket h), observed without claiming a ticket.  EMPTY is returned only
+  //     when Head is already park_limit tickets ahead of Tail, i.e. enough dequeuers are
+  //     parked (D2) to absorb the next enqueues; below that the caller claims a ticket.
+  //  D2 bounded parking.  A dequeuer whose slot is still vacant (its enqueuer has not
+  //     installed yet, or has not even claimed ticket h yet) re-reads its OWN slot with
+  //     __nanosleep backoff for at most park_ns before it invalidates the slot as L186-188
+  //     prescribe.  The wait is on a private address, so parked threads put no load on the
+  //     hot Head/Tail/Threshold lines, Head does not run away from Tail, and the enqueuer
+  //     that later draws ticket h hands its item straight to the parked dequeuer.  Pure delay
+  //     in front of the paper's steps: every operation still finishes in bounded own steps.
   template <class Finalize>
   __device__ __forceinline__ static int try_deq(const RingView& r, uint32_t* x, uint64_t* h_out, const Finalize& fin,
                                                 bool probe = false, uint32_t flags = 0) {
     const int64_t thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
     if (thr < 0) return RING_EMPTY;                                   // L166-169
+    const uint32_t park_ns = (flags & kNoDeqSpin) ? 0u : r.park_ns;
     if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {       // D1
       const uint64_t H = counter(ld_acquire(r.head));
-      if (counter(ld_relaxed(r.tail)) <= H) return RING_EMPTY;
+      const uint64_t T = counter(ld_relaxed(r.tail));
+      if (T + (park_ns ? r.park_limit : 0u) <= H) return RING_EMPTY;
     }
     const uint64_t h = take(r.head);                                  // L172
     *h_out = h;
     const uint32_t j = slot_of(r, h), c = cycle_of(r, h);             // L175
     uint64_t* sp = slot(r, j);
-    int spin = (flags & kNoDeqSpin) ? 0 : kDeqSpin;
+    uint32_t waited = 0, nap = 64;
     for (;;) {
       const uint64_t E = ld_acquire(sp);                              // L176 (acquire: payload edge, G15)
       if (F::cycle(E) == c && !F::vacant(E)) {                        // L178
@@ -206,8 +214,9 @@ struct Ring {
         return RING_OK;                                               // L182
       }
       if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
-        if (spin > 0 && F::vacant(E) && counter(ld_relaxed(r.tail)) > h) {   // D2
-          --spin; __nanosleep(64); continue;
+        if (waited < park_ns && F::vacant(E)) {                       // D2
+          __nanosleep(nap); waited += nap; nap = nap < 2048 ? nap * 2 : 2048;
+          continue;
         }
         const uint64_t New = F::vacant(E) ? F::advanced(E, c)         // L186-188
                                           : F::unsafe(E);             // L193

@@ -15,6 +15,8 @@ namespace gq {
 struct thread_ctx {
   uint32_t tid;          // unique per participating thread, < max_threads (record index for G-WFQ / YMC)
   uint32_t hungry = 0;   // bit 0: last dequeue came back EMPTY, bit 1: last enqueue came back FULL (probe hint, D1)
+  uint32_t help_cd = 0;  // G-WFQ / YMC: operations until the next peer inspection (help delay D)
+  uint32_t help_peer = 0;// next peer record to inspect
 };
 
 enum : int { OK = 0, FULL = 1, EMPTY = 2 };   // == GQ_OK / GQ_FULL / GQ_EMPTY of gq.h

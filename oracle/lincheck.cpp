@@ -259,14 +259,60 @@ int poly_check(const std::vector<Op>& h, std::string* why) {
       if (a.second && b.second && precedes(*b.second, *a.second))
         return fail("order: " + std::to_string(b.first->arg) + " dequeued before earlier-enqueued " + std::to_string(a.first->arg));
     }
-  for (const Op& d : h) {
-    if (d.op != OP_DEQ || d.status != ST_EMPTY) continue;
-    for (auto& v : vals)
-      if (precedes(*v.first, d) && (!v.second || precedes(d, *v.second)))
-        return fail("empty: EMPTY returned while value " + std::to_string(v.first->arg) + " was certainly in the queue");
+  // empty: DEQ->EMPTY d is impossible iff its whole interval is covered by values that are
+  // certainly in the queue: a chain x1..xk with enq(x1) finished before d began, enq(x_{i+1})
+  // finished before deq(x_i) began (x_{i+1} is in before x_i can leave), and deq(x_k) begun
+  // after d ended (or never).  Reachability over "enq(y) precedes deq(x)" edges.
+  const size_t nv = vals.size();
+  std::vector<std::vector<uint32_t>> succ(nv);
+  bool any_empty = false;
+  for (const Op& d : h) if (d.op == OP_DEQ && d.status == ST_EMPTY) any_empty = true;
+  if (any_empty) {
+    for (size_t x = 0; x < nv; ++x)
+      for (size_t y = 0; y < nv; ++y)
+        if (x != y && (!vals[x].second || precedes(*vals[y].first, *vals[x].second))) succ[x].push_back((uint32_t)y);
+    for (const Op& d : h) {
+      if (d.op != OP_DEQ || d.status != ST_EMPTY) continue;
+      std::vector<char> seen(nv, 0);
+      std::vector<uint32_t> stack;
+      for (size_t x = 0; x < nv; ++x)
+        if (precedes(*vals[x].first, d)) { seen[x] = 1; stack.push_back((uint32_t)x); }
+      while (!stack.empty()) {
+        const uint32_t x = stack.back(); stack.pop_back();
+        if (!vals[x].second || precedes(d, *vals[x].second))
+          return fail("empty: EMPTY returned although the queue held a value throughout the dequeue (chain ends at " +
+                      std::to_string(vals[x].first->arg) + ")");
+        // x leaves during or before d: only values certainly in before x can leave AND still
+        // relevant (their enqueue precedes x's dequeue) extend the cover
+        for (uint32_t y : succ[x]) if (!seen[y]) { seen[y] = 1; stack.push_back(y); }
+      }
+    }
   }
   if (why) why->clear();
   return LIN_OK;
+}
+
+// ---------------------------------------------------------------- capacity bound
+// Necessary condition for the bound |S| <= n: in every linearization, at time t every OK enqueue
+// that finished before t is in and no OK dequeue invoked after t is, so
+// |S(t)| >= #enqOK(end < t) - #deqOK(call <= t).  That lower bound must never exceed n.
+std::string capacity_check(const std::vector<Op>& h, uint64_t capacity) {
+  std::vector<std::pair<uint64_t, int>> ev;   // (time, +1 enq finished [counts for t > end] / -1 deq invoked)
+  for (const Op& o : h) {
+    if (o.status != ST_OK) continue;
+    if (o.op == OP_ENQ) ev.emplace_back(o.end + 1, +1);   // strictly after its end
+    else ev.emplace_back(o.call, -1);
+  }
+  std::sort(ev.begin(), ev.end(), [](const std::pair<uint64_t, int>& a, const std::pair<uint64_t, int>& b) {
+    return a.first != b.first ? a.first < b.first : a.second < b.second;   // dequeues first at equal time
+  });
+  int64_t lb = 0;
+  for (auto& e : ev) {
+    lb += e.second;
+    if (lb > (int64_t)capacity)
+      return "capacity: at t=" + std::to_string(e.first) + " at least " + std::to_string(lb) + " items must be in a queue of " + std::to_string(capacity);
+  }
+  return "";
 }
 
 // ---------------------------------------------------------------- conservation

@@ -11,8 +11,11 @@
 //                 precedence and replay it on FifoModel.  Tiny histories only.
 //   wgl_check   : Wing-Gong search with Lowe's memoisation (the algorithm family
 //                 PAPER.md ref [16] / Porcupine uses).  Exact; has a step budget.
-//   poly_check  : unique-value FIFO "bad pattern" test, O(m^2).  Exact for complete
-//                 histories whose operations all return OK; a sound refuter otherwise.
+//   poly_check  : unique-value FIFO "bad pattern" test (fresh / repeat / order / empty-witness),
+//                 polynomial.  Exact for complete histories of the UNBOUNDED FIFO (OK and
+//                 EMPTY returns); FULL returns and the capacity bound are outside it
+//                 (capacity_check gives the necessary condition), so with those it is a
+//                 sound refuter.
 //
 // Precedence (reading H2): A precedes B iff A.end < B.call strictly.
 // ret_status: 0 OK, 1 FULL (enqueue only), 2 EMPTY (dequeue only).
@@ -45,6 +48,9 @@ int wgl_check(const std::vector<Op>& h, uint64_t capacity, bool relaxed_full,
               uint64_t max_steps, uint64_t* steps_out);
 // returns LIN_VIOLATION with a reason, or LIN_OK meaning "no bad pattern found".
 int poly_check(const std::vector<Op>& h, std::string* why);
+
+// Necessary condition for the capacity bound (lower bound on |S(t)| over all linearizations).
+std::string capacity_check(const std::vector<Op>& h, uint64_t capacity);
 
 // Conservation / token protocol of PAPER.md L336: (i) exactly once, (ii) no value that
 // was never enqueued, (iii) per-producer order: values enqueued by one proc are dequeued

@@ -71,6 +71,13 @@ int orc_conservation(uint64_t m, const uint32_t* proc, const uint32_t* op, const
   return s.empty() ? 1 : 0;
 }
 
+int orc_capacity(uint64_t m, const uint32_t* proc, const uint32_t* op, const uint32_t* arg, const uint32_t* status,
+                 const uint32_t* val, const uint64_t* call, const uint64_t* end, uint64_t capacity, char* msg, uint64_t msg_cap) {
+  std::string s = capacity_check(gather(m, proc, op, arg, status, val, call, end), capacity);
+  put_msg(msg, msg_cap, s);
+  return s.empty() ? 1 : 0;
+}
+
 // out[0..9] = succ_enq, succ_deq, full, empty, tot_enq, tot_deq, sum_enq, sum_deq, sum_left, left
 void orc_mutex_bench(int mode, uint32_t threads, uint64_t capacity, uint64_t prefill, double producer_fraction,
                      uint64_t seed, double warmup_ms, double duration_ms, uint64_t* out, double* meas_seconds) {

@@ -32,7 +32,8 @@ class GqError(RuntimeError):
 class gq_opts(C.Structure):
     _fields_ = [("max_threads", C.c_uint32), ("enq_patience", C.c_uint32), ("deq_patience", C.c_uint32),
                 ("help_delay", C.c_uint32), ("ymc_pool_cells", C.c_uint64), ("storage", C.c_void_p),
-                ("storage_bytes", C.c_size_t), ("layout", C.c_uint32), ("flags", C.c_uint32)]
+                ("storage_bytes", C.c_size_t), ("layout", C.c_uint32), ("flags", C.c_uint32),
+                ("park_ns", C.c_uint32), ("_reserved", C.c_uint32)]
 
 
 class gq_run_cfg(C.Structure):

@@ -32,7 +32,7 @@ static int cuda_fail(cudaError_t e, const char* what) {
 extern "C" const char* gq_last_cuda_error(void) { return g_err; }
 extern "C" const char* gq_version(void) { return "gq 0.1 (sm_100a)"; }
 
-static_assert(sizeof(gq_opts) == 48 && sizeof(gq_run_cfg) == 64 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
+static_assert(sizeof(gq_opts) == 56 && sizeof(gq_run_cfg) == 64 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
               "ABI structs: the Python binding mirrors these layouts");
 
 // ------------------------------------------------------------------------------- handle
@@ -72,9 +72,10 @@ static constexpr size_t kHotStride = 1024;
 struct Layout {
   uint64_t N = 0;
   uint32_t order = 0, slot_shift = 0;
-  size_t off_hot = 0, off_aq = 0, off_fq = 0, off_data = 0, off_owner_aq = 0, off_owner_fq = 0, off_rec = 0, off_pool = 0;
+  size_t off_hot = 0, off_aq = 0, off_fq = 0, off_data = 0, off_owner_aq = 0, off_owner_fq = 0, off_rec = 0, off_rec_fq = 0, off_pool = 0;
   size_t total = 0;
   uint64_t pool_cells = 0;
+  uint32_t park_ns = 0;
 };
 
 template <class Q> static int max_blocks_per_sm(int block_threads);
@@ -88,6 +89,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   uint32_t k = o->max_threads ? o->max_threads : default_max_threads(kind);
   if (k == 0) k = 148 * 2048;                         // no device visible: size for a full B200
   *max_threads_out = k;
+  L->park_ns = o->park_ns ? o->park_ns : 250000u;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
   if (kind == GQ_LFQ || kind == GQ_WFQ) {
@@ -105,6 +107,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
       L->off_owner_aq = off; off += (size_t)(2 * L->N) * 8;
       L->off_owner_fq = off; off += (size_t)(2 * L->N) * 8;
       L->off_rec = off; off += (size_t)k * sizeof(WfqRecord);
+      L->off_rec_fq = off; off += (size_t)k * sizeof(WfqRecord);
     }
   } else {
     L->pool_cells = o->ymc_pool_cells ? o->ymc_pool_cells : (1ull << 26);
@@ -140,17 +143,30 @@ __global__ void format_ring_kernel(RingView r, uint64_t slots, uint64_t count) {
   }
 }
 
-static RingView make_ring(char* base, const Layout& L, size_t off_entries, size_t off_owner, int hot_slot) {
+static RingView make_ring(char* base, const Layout& L, size_t off_entries, size_t off_owner, int hot_slot, size_t off_rec = 0) {
   RingView r{};
   r.entry = reinterpret_cast<uint64_t*>(base + off_entries);
   r.head = reinterpret_cast<uint64_t*>(base + L.off_hot + (hot_slot + 0) * kHotStride);
   r.tail = reinterpret_cast<uint64_t*>(base + L.off_hot + (hot_slot + 1) * kHotStride);
   r.threshold = reinterpret_cast<int64_t*>(base + L.off_hot + (hot_slot + 2) * kHotStride);
   r.owner = off_owner ? reinterpret_cast<uint64_t*>(base + off_owner) : nullptr;
+  r.rec = off_rec ? base + off_rec : nullptr;
   r.thr_reset = (int64_t)(3 * L.N - 1);
   r.order = L.order;
   r.slot_shift = L.slot_shift;
+  r.park_ns = L.park_ns;
+  r.park_limit = (uint32_t)std::min<uint64_t>(L.N / 2, 0x7FFFFFFFu);
   return r;
+}
+
+// G-WFQ per-thread records: everything zero, sequence pairs apart (seq1 = 1, seq2 = 0) so that no
+// helper accepts an unpublished record.
+__global__ void format_wfq_records_kernel(WfqRecord* rec, uint32_t n) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  WfqRecord z{};
+  z.seq1 = 1; z.p2_seq1 = 1;
+  rec[i] = z;
 }
 
 static int format_queue(gq_queue* q, cudaStream_t st) {
@@ -159,6 +175,12 @@ static int format_queue(gq_queue* q, cudaStream_t st) {
   if (q->kind == GQ_LFQ) {
     format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.aq, slots, 0);
     format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.fq, slots, q->capacity);
+  } else if (q->kind == GQ_WFQ) {
+    format_ring_kernel<WfqFmt><<<grd, blk, 0, st>>>(q->wfq.aq, slots, 0);
+    format_ring_kernel<WfqFmt><<<grd, blk, 0, st>>>(q->wfq.fq, slots, q->capacity);
+    const unsigned g2 = (q->max_threads + blk - 1) / blk;
+    format_wfq_records_kernel<<<g2, blk, 0, st>>>(static_cast<WfqRecord*>(q->wfq.aq.rec), q->max_threads);
+    format_wfq_records_kernel<<<g2, blk, 0, st>>>(static_cast<WfqRecord*>(q->wfq.fq.rec), q->max_threads);
   } else {
     return GQ_E_INVAL;
   }
@@ -176,6 +198,7 @@ static int max_blocks_per_sm(int block_threads) {
 static int kind_blocks_per_sm(int kind, int block_threads) {
   switch (kind) {
     case GQ_LFQ: return max_blocks_per_sm<LfqView>(block_threads);
+    case GQ_WFQ: return max_blocks_per_sm<WfqView>(block_threads);
     default: return 0;
   }
 }
@@ -225,6 +248,17 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
     q->lfq.data = reinterpret_cast<uint32_t*>(q->base + L.off_data);
     q->lfq.capacity = (uint32_t)capacity;
     q->lfq.flags = q->opts.flags;
+  } else if (kind == GQ_WFQ) {
+    q->wfq.aq = make_ring(q->base, L, L.off_aq, L.off_owner_aq, 0, L.off_rec);
+    q->wfq.fq = make_ring(q->base, L, L.off_fq, L.off_owner_fq, 3, L.off_rec_fq);
+    q->wfq.data = reinterpret_cast<uint32_t*>(q->base + L.off_data);
+    q->wfq.capacity = (uint32_t)capacity;
+    q->wfq.nthreads = k;
+    auto pat = [](uint32_t v, uint32_t dflt) { return v == GQ_PATIENCE_ZERO ? 0u : (v ? v : dflt); };
+    q->wfq.enq_patience = pat(q->opts.enq_patience, 16);      // reading W2
+    q->wfq.deq_patience = pat(q->opts.deq_patience, 64);
+    q->wfq.help_delay = q->opts.help_delay ? q->opts.help_delay : 64;   // D = 64
+    q->wfq.flags = q->opts.flags;
   }
   rc = format_queue(q, nullptr);
   if (rc == 0) { cudaError_t e2 = cudaDeviceSynchronize(); if (e2 != cudaSuccess) rc = cuda_fail(e2, "format"); }
@@ -264,6 +298,43 @@ extern "C" int queue_device_view(const gq_queue* q, void* view_out, size_t view_
   }
   if (view_bytes < n) return GQ_E_INVAL;
   std::memcpy(view_out, src, n);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------- kind dispatch
+template <class Fn>
+static int dispatch(gq_queue* q, Fn&& fn) {
+  switch (q->kind) {
+    case GQ_LFQ: return fn(q->lfq);
+    case GQ_WFQ: return fn(q->wfq);
+    default: return GQ_E_INVAL;
+  }
+}
+static void set_nthreads(LfqView&, uint32_t) {}
+static void set_nthreads(WfqView& v, uint32_t n) { v.nthreads = n; }
+static void set_nthreads(YmcView& v, uint32_t n) { v.nthreads = n; }
+
+// slow-path statistics live in the per-thread records; sum and clear them after a run
+__global__ void wfq_stats_kernel(WfqRecord* a, WfqRecord* b, uint32_t n, uint64_t* out) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  uint64_t se = 0, sd = 0, hp = 0;
+  if (i < n) {
+    se = a[i].n_slow_enq + b[i].n_slow_enq; sd = a[i].n_slow_deq + b[i].n_slow_deq; hp = a[i].n_helps + b[i].n_helps;
+    a[i].n_slow_enq = a[i].n_slow_deq = a[i].n_helps = 0;
+    b[i].n_slow_enq = b[i].n_slow_deq = b[i].n_helps = 0;
+  }
+  se = warp_sum(se); sd = warp_sum(sd); hp = warp_sum(hp);
+  if ((threadIdx.x & 31) == 0) { if (se) red_add_relaxed(out, se); if (sd) red_add_relaxed(out + 1, sd); if (hp) red_add_relaxed(out + 2, hp); }
+}
+static int collect_stats(gq_queue* q, gq_run_result* res) {
+  if (q->kind != GQ_WFQ) return 0;
+  uint64_t* d = nullptr; uint64_t h[3] = {0, 0, 0};
+  CU(cudaMalloc(&d, 24)); cudaMemset(d, 0, 24);
+  wfq_stats_kernel<<<(q->max_threads + 255) / 256, 256>>>(static_cast<WfqRecord*>(q->wfq.aq.rec), static_cast<WfqRecord*>(q->wfq.fq.rec), q->max_threads, d);
+  cudaError_t e = cudaMemcpy(h, d, 24, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return cuda_fail(e, "stats");
+  res->slow_enq = h[0]; res->slow_deq = h[1]; res->helps = h[2];
   return 0;
 }
 
@@ -354,6 +425,7 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   CU(cudaMemset(q->d_ctr, 0, C_COUNT * sizeof(uint64_t)));
   BenchParams p = make_params(cfg, r, mode);
   Q v = view;
+  set_nthreads(v, r.threads);          // help ring = the launched threads (reading W7)
   uint64_t* ctr = q->d_ctr; gq_hist_rec* h = q->d_hist;
   void* args[] = {&v, &p, &ctr, &h};
   cudaEvent_t e0, e1;
@@ -365,16 +437,14 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + 60.0);
   if (rc == 0) rc = finish_run(q->d_ctr, e0, e1, cfg, r, res);
   cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (rc == 0) rc = collect_stats(q, res);
   if (rc == 0 && res->pool_exhausted) return GQ_E_POOL;
   return rc;
 }
 
 static int run_bench(gq_queue* q, const gq_run_cfg* cfg, int mode, gq_run_result* res) {
   if (!q || !cfg || !res) return GQ_E_INVAL;
-  switch (q->kind) {
-    case GQ_LFQ: return run_bench_t<LfqView>(q, q->lfq, cfg, mode, res);
-    default: return GQ_E_INVAL;
-  }
+  return dispatch(q, [&](auto& view) { return run_bench_t(q, view, cfg, mode, res); });
 }
 extern "C" int run_balanced(gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res) { return run_bench(q, cfg, MODE_BALANCED, res); }
 extern "C" int run_split(gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res) { return run_bench(q, cfg, MODE_SPLIT, res); }
@@ -468,10 +538,7 @@ extern "C" int queue_prefill(gq_queue* q, const uint32_t* host_vals, uint64_t co
   if (!q || (!host_vals && count)) return GQ_E_INVAL;
   if (count == 0) return 0;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  switch (q->kind) {
-    case GQ_LFQ: return prefill_t<LfqView>(q->lfq, host_vals, count, st);
-    default: return GQ_E_INVAL;
-  }
+  return dispatch(q, [&](auto& view) { return prefill_t(view, host_vals, count, st); });
 }
 
 template <class Q>
@@ -494,10 +561,7 @@ static int drain_t(const Q& view, uint32_t* host_out, uint64_t max, uint64_t* n_
 extern "C" int queue_drain(gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream) {
   if (!q || !n_out || (!host_out && max)) return GQ_E_INVAL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  switch (q->kind) {
-    case GQ_LFQ: return drain_t<LfqView>(q->lfq, host_out, max, n_out, st);
-    default: return GQ_E_INVAL;
-  }
+  return dispatch(q, [&](auto& view) { return drain_t(view, host_out, max, n_out, st); });
 }
 
 template <class Q>
@@ -517,10 +581,7 @@ extern "C" int queue_run_script(gq_queue* q, const uint32_t* host_op, const uint
                                 uint32_t tid, uint32_t* host_status, uint32_t* host_val) {
   if (!q || !host_op || !host_arg || !host_status || !host_val || tid >= q->max_threads) return GQ_E_INVAL;
   if (count == 0) return 0;
-  switch (q->kind) {
-    case GQ_LFQ: return script_t<LfqView>(q->lfq, host_op, host_arg, count, tid, host_status, host_val);
-    default: return GQ_E_INVAL;
-  }
+  return dispatch(q, [&](auto& view) { return script_t(view, host_op, host_arg, count, tid, host_status, host_val); });
 }
 
 extern "C" int history_dump(gq_queue* q, gq_hist_rec* host_out, uint64_t max, uint64_t* n_out) {

@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(512) bench_kernel(Q q, BenchParams p, uint64_t
 
   if (tid < p.threads) {
     thread_ctx ctx{tid};
+    ctx.help_peer = tid + 1;
     bool do_enq = true, do_deq = true;
     if (p.mode == MODE_SPLIT) {
       do_enq = (uint64_t)mix32(p.seed * 0x9e3779b9u + tid) < p.prod_threshold;

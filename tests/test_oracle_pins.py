@@ -216,3 +216,47 @@ def test_mutex_baseline_conserves(mode, prefill, p):
     assert (r["sum_enq"] - r["sum_deq"] - r["sum_left"]) % 2**64 == 0
     assert r["left"] <= 1024
     assert r["succ_enq"] + r["succ_deq"] > 0 and r["mops"] > 0
+
+
+# ------------------------------------------------------------------ poly == definition on OK/EMPTY histories
+def test_poly_equals_brute_force_without_capacity():
+    """With no FULL returns and no capacity bound, the four bad patterns (fresh, repeat, order,
+    empty-witness chain) are an exact characterisation: compare with brute force both ways."""
+    agree_ok = agree_bad = 0
+    for seed in range(4000):
+        procs = 2 + seed % 3
+        rows, _ = gen_history(50_000 + seed, procs, 4 + seed % 6, 10**9, p_enq=0.45)
+        cands = [rows, mutate(rows, seed), mutate(mutate(rows, seed), seed + 1)]
+        for m in cands:
+            hm = H(m)
+            if oracle.precheck(hm):
+                continue
+            truth = oracle.brute(hm, 10**9)
+            pr, why = oracle.poly(hm)
+            assert pr == truth, (seed, m, why)
+            agree_ok += truth == LIN_OK
+            agree_bad += truth == LIN_VIOLATION
+    assert agree_ok > 3000 and agree_bad > 1000
+
+
+def test_empty_witness_chain_longer_than_one():
+    # x in queue from t=1; y enqueued (t 2..3) before x is dequeued (t 6..7); y dequeued only after
+    # the EMPTY dequeue (t 4..9) ended: no instant inside [4, 9] at which the queue is empty.
+    rows = [(0, E, 1, 0, 0, 0, 1), (1, E, 2, 0, 0, 2, 3), (2, D, 0, ST_EMPTY, 0, 4, 9),
+            (3, D, 0, 0, 1, 6, 7), (3, D, 0, 0, 2, 10, 11)]
+    assert oracle.brute(H(rows), 8) == LIN_VIOLATION
+    assert oracle.poly(H(rows))[0] == LIN_VIOLATION
+    # same, but y's enqueue overlaps x's dequeue: the queue may be empty in between
+    rows2 = [(0, E, 1, 0, 0, 0, 1), (1, E, 2, 0, 0, 2, 8), (2, D, 0, ST_EMPTY, 0, 4, 9),
+             (3, D, 0, 0, 1, 6, 7), (3, D, 0, 0, 2, 10, 11)]
+    assert oracle.brute(H(rows2), 8) == LIN_OK
+    assert oracle.poly(H(rows2))[0] == LIN_OK
+
+
+def test_capacity_lower_bound():
+    rows = [(0, E, 1, 0, 0, 0, 1), (1, E, 2, 0, 0, 0, 1), (2, E, 3, 0, 0, 2, 3)]
+    assert oracle.capacity_bound(H(rows), 3) == ""
+    assert "capacity" in oracle.capacity_bound(H(rows), 2)
+    # a dequeue invoked before the third enqueue finished may have made room
+    rows2 = rows + [(3, D, 0, 0, 1, 3, 5)]
+    assert oracle.capacity_bound(H(rows2), 2) == ""
