@@ -17,6 +17,7 @@ struct thread_ctx {
   uint32_t hungry = 0;   // bit 0: last dequeue came back EMPTY, bit 1: last enqueue came back FULL (probe hint, D1)
   uint32_t help_cd = 0;  // G-WFQ / YMC: operations until the next peer inspection (help delay D)
   uint32_t help_peer = 0;// next peer record to inspect
+  uint64_t last_ticket = 0;  // ticket (AQ head ticket / YMC cell) of the last successful dequeue: FIFO position
 };
 
 enum : int { OK = 0, FULL = 1, EMPTY = 2 };   // == GQ_OK / GQ_FULL / GQ_EMPTY of gq.h
@@ -33,12 +34,12 @@ namespace detail {
 
 template <class F, bool kUniform, bool kWarpFaa, class Fin>
 __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, uint64_t* retries, const Fin& fin,
-                                             bool probe, uint32_t flags) {
+                                             bool probe, uint32_t flags, uint64_t* ticket = nullptr) {
   Backoff bo;
   for (;;) {
     uint64_t h;
     const int s = Ring<F, kUniform, kWarpFaa>::try_deq(r, idx, &h, fin, probe, flags);
-    if (s != RING_RETRY) return s;
+    if (s != RING_RETRY) { if (ticket) *ticket = h; return s; }
     ++*retries;
     probe = true;
     bo.pause();
@@ -78,7 +79,7 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   uint32_t idx;
-  if (ring_deq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, &idx, retries, NoFinalize{}, (ctx.hungry & 1u) != 0, q.flags) == RING_EMPTY) {
+  if (ring_deq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, &idx, retries, NoFinalize{}, (ctx.hungry & 1u) != 0, q.flags, &ctx.last_ticket) == RING_EMPTY) {
     ctx.hungry |= 1u;
     return EMPTY;
   }

@@ -274,13 +274,13 @@ struct Wf {
 
   template <bool kUniform, bool kWarpFaa>
   __device__ static int ring_deq(const RingView& r, uint32_t* x, uint32_t patience, uint32_t me, uint32_t nthreads,
-                                 uint64_t* retries, bool probe, uint32_t flags) {
+                                 uint64_t* retries, bool probe, uint32_t flags, uint64_t* ticket = nullptr) {
     const Finalize fin{nthreads};
     uint64_t h = 0;
     bool have_h = false;
     for (uint32_t p = 0; p < patience; ++p) {
       const int s = Ring<F, kUniform, kWarpFaa>::try_deq(r, x, &h, fin, probe, flags);
-      if (s != RING_RETRY) return s;
+      if (s != RING_RETRY) { if (ticket) *ticket = h; return s; }
       have_h = true; probe = true;
       ++*retries;
     }
@@ -302,6 +302,7 @@ struct Wf {
     // result of a slow dequeue (reading W9): the slot named by the final localHead
     using R = Ring<F, kUniform, kWarpFaa>;
     const uint64_t H = ld_acquire(&my->localHead) >> S;
+    if (ticket) *ticket = H;
     const uint32_t j = R::slot_of(r, H), c = R::cycle_of(r, H);
     uint64_t* sp = R::slot(r, j);
     const uint64_t E = ld_acquire(sp);
@@ -351,7 +352,7 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   wfq_help_threads(q, ctx);
   uint32_t idx;
-  if (Wf::ring_deq<kUniform, kWarpFaa>(q.aq, &idx, q.deq_patience, ctx.tid, q.nthreads, retries, (ctx.hungry & 1u) != 0, q.flags) == RING_EMPTY) {
+  if (Wf::ring_deq<kUniform, kWarpFaa>(q.aq, &idx, q.deq_patience, ctx.tid, q.nthreads, retries, (ctx.hungry & 1u) != 0, q.flags, &ctx.last_ticket) == RING_EMPTY) {
     ctx.hungry |= 1u;
     return EMPTY;
   }

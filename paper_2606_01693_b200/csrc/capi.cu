@@ -51,6 +51,8 @@ struct gq_queue {
   uint64_t* d_ctr = nullptr;        // C_COUNT result counters
   gq_hist_rec* d_hist = nullptr;
   uint64_t hist_cap = 0, hist_n = 0;
+  bool formatted = false;
+  bool fresh = false;      // formatted and not operated on since: the fast path cannot fail (queue_prefill)
 };
 
 static int g_sms = 0;
@@ -110,7 +112,9 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
       L->off_rec_fq = off; off += (size_t)k * sizeof(WfqRecord);
     }
   } else {
-    L->pool_cells = o->ymc_pool_cells ? o->ymc_pool_cells : (1ull << 26);
+    L->pool_cells = o->ymc_pool_cells ? o->ymc_pool_cells : (1ull << 26);    // reading Y3
+    if (L->pool_cells < 64 || L->pool_cells >= (1ull << 40)) return GQ_E_INVAL;
+    L->N = pow2ceil(k);
     L->off_rec = off; off += (size_t)k * sizeof(YmcHandle);
     L->off_pool = off; off += (size_t)L->pool_cells * sizeof(YmcCell);
   }
@@ -169,7 +173,41 @@ __global__ void format_wfq_records_kernel(WfqRecord* rec, uint32_t n) {
   rec[i] = z;
 }
 
+// G-WFQ-YMC: handles with no request published, helping pointers at the next thread (reading Y6).
+__global__ void format_ymc_handles_kernel(YmcHandle* h, uint32_t n) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  YmcHandle z{};
+  z.enq_help_id = Ymc::kNoId;
+  z.enq_peer = z.deq_peer = i + 1 < n ? i + 1 : 0;
+  h[i] = z;
+}
+// T = H = 0, flag clear, and the sentinel cell at the end of the pool sealed (val = top, enq = top_e,
+// deq = top_d) so that a ticket past the pool can never deposit or claim anything.
+__global__ void format_ymc_words_kernel(YmcView q) {
+  *q.tail = 0; *q.head = 0; *q.exhausted = 0;
+  YmcCell* c = q.pool + (q.pool_cells - 1);
+  c->val = Ymc::kTop; c->enq = Ymc::kTop32; c->deq = Ymc::kTop32;
+}
+
 static int format_queue(gq_queue* q, cudaStream_t st) {
+  if (q->kind == GQ_WFQ_YMC) {
+    // only the cells tickets have reached can be dirty: zero [0, max(T, H) + k + 64)
+    uint64_t dirty = q->ymc.pool_cells;
+    if (q->formatted) {
+      uint64_t th[2] = {0, 0};
+      CU(cudaMemcpyAsync(&th[0], q->ymc.tail, 8, cudaMemcpyDeviceToHost, st));
+      CU(cudaMemcpyAsync(&th[1], q->ymc.head, 8, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      dirty = std::min<uint64_t>(q->ymc.pool_cells, std::max(th[0], th[1]) + q->max_threads + 64);
+    }
+    CU(cudaMemsetAsync(q->ymc.pool, 0, (size_t)dirty * sizeof(YmcCell), st));
+    format_ymc_handles_kernel<<<(q->max_threads + 255) / 256, 256, 0, st>>>(q->ymc.handles, q->max_threads);
+    format_ymc_words_kernel<<<1, 1, 0, st>>>(q->ymc);
+    CU(cudaGetLastError());
+    q->formatted = true;
+    return 0;
+  }
   const uint64_t slots = 2 * q->N;
   const unsigned blk = 256, grd = (unsigned)((slots + blk - 1) / blk);
   if (q->kind == GQ_LFQ) {
@@ -199,6 +237,7 @@ static int kind_blocks_per_sm(int kind, int block_threads) {
   switch (kind) {
     case GQ_LFQ: return max_blocks_per_sm<LfqView>(block_threads);
     case GQ_WFQ: return max_blocks_per_sm<WfqView>(block_threads);
+    case GQ_WFQ_YMC: return max_blocks_per_sm<YmcView>(block_threads);
     default: return 0;
   }
 }
@@ -259,8 +298,24 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
     q->wfq.deq_patience = pat(q->opts.deq_patience, 64);
     q->wfq.help_delay = q->opts.help_delay ? q->opts.help_delay : 64;   // D = 64
     q->wfq.flags = q->opts.flags;
+  } else {
+    auto pat = [](uint32_t v, uint32_t dflt) { return v == GQ_PATIENCE_ZERO ? 0u : (v ? v : dflt); };
+    q->ymc.pool = reinterpret_cast<YmcCell*>(q->base + L.off_pool);
+    q->ymc.pool_cells = L.pool_cells;
+    q->ymc.head = reinterpret_cast<uint64_t*>(q->base + L.off_hot + 0 * kHotStride);
+    q->ymc.tail = reinterpret_cast<uint64_t*>(q->base + L.off_hot + 1 * kHotStride);
+    q->ymc.exhausted = reinterpret_cast<uint64_t*>(q->base + L.off_hot + 2 * kHotStride);
+    q->ymc.handles = reinterpret_cast<YmcHandle*>(q->base + L.off_rec);
+    q->ymc.nthreads = k;
+    q->ymc.enq_patience = pat(q->opts.enq_patience, 10);      // reading Y8
+    q->ymc.deq_patience = pat(q->opts.deq_patience, 10);
+    q->ymc.help_delay = q->opts.help_delay ? q->opts.help_delay : 1;   // [5]: after every successful dequeue
+    q->ymc.flags = q->opts.flags;
+    q->ymc.park_ns = L.park_ns;
+    q->ymc.park_limit = (uint32_t)std::min<uint64_t>(L.N / 2, 0x7FFFFFFFu);
   }
   rc = format_queue(q, nullptr);
+  q->fresh = rc == 0;
   if (rc == 0) { cudaError_t e2 = cudaDeviceSynchronize(); if (e2 != cudaSuccess) rc = cuda_fail(e2, "format"); }
   if (rc) { queue_destroy(q); return rc; }
   *out = q;
@@ -283,6 +338,7 @@ extern "C" int queue_reset(gq_queue* q, void* stream) {
   int rc = format_queue(q, st);
   if (rc) return rc;
   CU(cudaStreamSynchronize(st));
+  q->fresh = true;
   return 0;
 }
 
@@ -307,6 +363,7 @@ static int dispatch(gq_queue* q, Fn&& fn) {
   switch (q->kind) {
     case GQ_LFQ: return fn(q->lfq);
     case GQ_WFQ: return fn(q->wfq);
+    case GQ_WFQ_YMC: return fn(q->ymc);
     default: return GQ_E_INVAL;
   }
 }
@@ -326,12 +383,28 @@ __global__ void wfq_stats_kernel(WfqRecord* a, WfqRecord* b, uint32_t n, uint64_
   se = warp_sum(se); sd = warp_sum(sd); hp = warp_sum(hp);
   if ((threadIdx.x & 31) == 0) { if (se) red_add_relaxed(out, se); if (sd) red_add_relaxed(out + 1, sd); if (hp) red_add_relaxed(out + 2, hp); }
 }
+__global__ void ymc_stats_kernel(YmcHandle* a, uint32_t n, uint64_t* out) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  uint64_t se = 0, sd = 0, hp = 0;
+  if (i < n) {
+    se = a[i].n_slow_enq; sd = a[i].n_slow_deq; hp = a[i].n_helps;
+    a[i].n_slow_enq = a[i].n_slow_deq = a[i].n_helps = 0;
+  }
+  se = warp_sum(se); sd = warp_sum(sd); hp = warp_sum(hp);
+  if ((threadIdx.x & 31) == 0) { if (se) red_add_relaxed(out, se); if (sd) red_add_relaxed(out + 1, sd); if (hp) red_add_relaxed(out + 2, hp); }
+}
 static int collect_stats(gq_queue* q, gq_run_result* res) {
-  if (q->kind != GQ_WFQ) return 0;
-  uint64_t* d = nullptr; uint64_t h[3] = {0, 0, 0};
-  CU(cudaMalloc(&d, 24)); cudaMemset(d, 0, 24);
-  wfq_stats_kernel<<<(q->max_threads + 255) / 256, 256>>>(static_cast<WfqRecord*>(q->wfq.aq.rec), static_cast<WfqRecord*>(q->wfq.fq.rec), q->max_threads, d);
-  cudaError_t e = cudaMemcpy(h, d, 24, cudaMemcpyDeviceToHost);
+  if (q->kind == GQ_LFQ) return 0;
+  uint64_t* d = nullptr; uint64_t h[4] = {0, 0, 0, 0};
+  CU(cudaMalloc(&d, 32)); cudaMemset(d, 0, 32);
+  if (q->kind == GQ_WFQ)
+    wfq_stats_kernel<<<(q->max_threads + 255) / 256, 256>>>(static_cast<WfqRecord*>(q->wfq.aq.rec), static_cast<WfqRecord*>(q->wfq.fq.rec), q->max_threads, d);
+  else {
+    ymc_stats_kernel<<<(q->max_threads + 255) / 256, 256>>>(q->ymc.handles, q->max_threads, d);
+    cudaMemcpyAsync(d + 3, q->ymc.exhausted, 8, cudaMemcpyDeviceToDevice);
+  }
+  cudaError_t e = cudaMemcpy(h, d, 32, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess && h[3]) res->pool_exhausted = 1;
   cudaFree(d);
   if (e != cudaSuccess) return cuda_fail(e, "stats");
   res->slow_enq = h[0]; res->slow_deq = h[1]; res->helps = h[2];
@@ -444,6 +517,7 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
 
 static int run_bench(gq_queue* q, const gq_run_cfg* cfg, int mode, gq_run_result* res) {
   if (!q || !cfg || !res) return GQ_E_INVAL;
+  q->fresh = false;
   return dispatch(q, [&](auto& view) { return run_bench_t(q, view, cfg, mode, res); });
 }
 extern "C" int run_balanced(gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res) { return run_bench(q, cfg, MODE_BALANCED, res); }
@@ -520,14 +594,14 @@ extern "C" int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t se
 
 // ------------------------------------------------------------------------------- prefill / drain / script / history
 template <class Q>
-static int prefill_t(const Q& view, const uint32_t* host_vals, uint64_t count, cudaStream_t st) {
+static int prefill_t(const Q& view, const uint32_t* host_vals, uint64_t count, cudaStream_t st, uint32_t serial) {
   uint32_t* d_vals = nullptr; uint64_t* d_n = nullptr;
   CU(cudaMalloc(&d_vals, std::max<uint64_t>(count, 1) * 4));
   cudaError_t e = cudaMalloc(&d_n, 8);
   if (e != cudaSuccess) { cudaFree(d_vals); return cuda_fail(e, "cudaMalloc"); }
   uint64_t n_ok = 0;
   e = cudaMemcpyAsync(d_vals, host_vals, count * 4, cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess) { prefill_kernel<Q><<<1, 32, 0, st>>>(view, d_vals, count, d_n); e = cudaGetLastError(); }
+  if (e == cudaSuccess) { prefill_kernel<Q><<<1, 32, 0, st>>>(view, d_vals, count, d_n, serial); e = cudaGetLastError(); }
   if (e == cudaSuccess) e = cudaMemcpyAsync(&n_ok, d_n, 8, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d_vals); cudaFree(d_n);
@@ -538,7 +612,12 @@ extern "C" int queue_prefill(gq_queue* q, const uint32_t* host_vals, uint64_t co
   if (!q || (!host_vals && count)) return GQ_E_INVAL;
   if (count == 0) return 0;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  return dispatch(q, [&](auto& view) { return prefill_t(view, host_vals, count, st); });
+  // Lanes enqueue side by side only where ticket order is certain to be lane order: a freshly
+  // formatted queue on its fast path.  Anywhere else (holes left by abandoned tickets after a
+  // concurrent run, all-slow builds) the lanes take turns.
+  const uint32_t serial = !q->fresh || (q->kind != GQ_LFQ && q->opts.enq_patience == GQ_PATIENCE_ZERO);
+  q->fresh = false;
+  return dispatch(q, [&](auto& view) { return prefill_t(view, host_vals, count, st, serial); });
 }
 
 template <class Q>
@@ -561,6 +640,7 @@ static int drain_t(const Q& view, uint32_t* host_out, uint64_t max, uint64_t* n_
 extern "C" int queue_drain(gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream) {
   if (!q || !n_out || (!host_out && max)) return GQ_E_INVAL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  q->fresh = false;
   return dispatch(q, [&](auto& view) { return drain_t(view, host_out, max, n_out, st); });
 }
 
@@ -581,6 +661,7 @@ extern "C" int queue_run_script(gq_queue* q, const uint32_t* host_op, const uint
                                 uint32_t tid, uint32_t* host_status, uint32_t* host_val) {
   if (!q || !host_op || !host_arg || !host_status || !host_val || tid >= q->max_threads) return GQ_E_INVAL;
   if (count == 0) return 0;
+  q->fresh = false;
   return dispatch(q, [&](auto& view) { return script_t(view, host_op, host_arg, count, tid, host_status, host_val); });
 }
 

@@ -112,21 +112,42 @@ __global__ void __launch_bounds__(512) bench_kernel(Q q, BenchParams p, uint64_t
 }
 
 // ---- service kernels --------------------------------------------------------------------
-// One warp enqueues vals[0..count) in array order (quiescent queue: lane order = ticket order).
+// One warp enqueues vals[0..count) in array order.  On a quiescent queue the fast path succeeds
+// at the first ticket, so lane order = ticket order = FIFO order.  Two cases need care:
+//  - G-WFQ-YMC after EMPTY dequeues has H > T, and the cells in between are burnt (marked top):
+//    T is first advanced to H, which is what the failed tickets would do one by one;
+//  - all-slow builds (patience 0) place concurrent requests in any order, which is linearizable
+//    but not array order: `serial` makes the lanes take turns.
+__device__ __forceinline__ void prefill_prepare(const LfqView&) {}
+__device__ __forceinline__ void prefill_prepare(const WfqView&) {}
+__device__ __forceinline__ void prefill_prepare(const YmcView& q) { Ymc::advance(q.tail, ld_acquire(q.head)); }
+
 template <class Q>
-__global__ void prefill_kernel(Q q, const uint32_t* vals, uint64_t count, uint64_t* n_ok) {
+__global__ void prefill_kernel(Q q, const uint32_t* vals, uint64_t count, uint64_t* n_ok, uint32_t serial) {
   thread_ctx ctx{threadIdx.x};
   uint64_t ok = 0;
+  if (threadIdx.x == 0) prefill_prepare(q);
+  __syncwarp();
   for (uint64_t base = 0; base < count; base += 32) {
     const uint64_t i = base + threadIdx.x;
-    if (i < count && enqueue<true, true>(q, ctx, vals[i]) == OK) ++ok;
+    if (serial) {
+      for (uint32_t l = 0; l < 32; ++l) {
+        if (threadIdx.x == l && i < count && enqueue<false, true>(q, ctx, vals[i]) == OK) ++ok;
+        __syncwarp();
+      }
+    } else {
+      if (i < count && enqueue<true, true>(q, ctx, vals[i]) == OK) ++ok;
+    }
     __syncwarp();
   }
   ok = warp_sum(ok);
   if (threadIdx.x == 0) *n_ok = ok;
 }
 
-// One warp dequeues until EMPTY (or max) in FIFO order.
+// One warp dequeues until EMPTY (or max) in FIFO order.  Each round's values are written in the
+// order of the tickets they were dequeued at (thread_ctx::last_ticket: AQ head ticket / YMC
+// cell), not in lane order: a lane that met a hole left by an abandoned ticket retries at a
+// later ticket.  Rounds are sequential, so ticket order across rounds is round order.
 template <class Q>
 __global__ void drain_kernel(Q q, uint32_t* out, uint64_t max, uint64_t* n_out) {
   thread_ctx ctx{threadIdx.x};
@@ -139,7 +160,10 @@ __global__ void drain_kernel(Q q, uint32_t* out, uint64_t max, uint64_t* n_out) 
     if (threadIdx.x < want) s = dequeue<true, true>(q, ctx, &v);
     __syncwarp();
     const uint32_t okmask = __ballot_sync(0xffffffffu, s == OK);
-    if (s == OK) out[n + __popc(okmask & lanemask_lt())] = v;
+    const uint64_t mine = s == OK ? ctx.last_ticket : ~0ull;
+    uint32_t rank = 0;
+    for (int l = 0; l < 32; ++l) rank += __shfl_sync(0xffffffffu, mine, l) < mine;
+    if (s == OK) out[n + rank] = v;
     n += __popc(okmask);
     if (__popc(okmask) < (int)want) break;
   }

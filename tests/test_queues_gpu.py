@@ -21,11 +21,26 @@ VARIANTS = {
     "G-WFQ": (gq.GQ_WFQ, {}),
     "G-WFQ-p0": (gq.GQ_WFQ, dict(enq_patience=Z, deq_patience=Z, help_delay=1)),
     "G-WFQ-p1": (gq.GQ_WFQ, dict(enq_patience=1, deq_patience=1, help_delay=2)),
+    # G-WFQ-YMC: capacity does not throttle (reading Y3), so its model capacity is "unbounded";
+    # the pool is sized per test.  -p0: every enqueue takes the slow path, every dequeue makes one
+    # unparked attempt and then takes the slow path (reading Y8).
+    "G-WFQ-YMC": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22)),
+    "YMC-p0": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, enq_patience=Z, deq_patience=Z)),
+    "YMC-p1": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, enq_patience=1, deq_patience=1)),
 }
 KINDS = list(VARIANTS)          # every test below runs for each of these
 SMALL = KINDS                   # tiny / single-thread cases
-BIG = ["G-LFQ", "G-WFQ"]        # full-occupancy cases
+BIG = ["G-LFQ", "G-WFQ", "G-WFQ-YMC"]        # full-occupancy cases
 IDS = KINDS
+UNBOUNDED = 1 << 31
+
+
+def is_ymc(kind):
+    return VARIANTS[kind][0] == gq.GQ_WFQ_YMC
+
+
+def model_capacity(kind, capacity):
+    return UNBOUNDED if is_ymc(kind) else capacity
 
 
 def make(kind, capacity, **opts):
@@ -64,11 +79,11 @@ def test_single_thread_equals_model(kind, capacity):
         st, val = gq.queue_run_script(q, ops, args, tid=5)
     finally:
         gq.queue_destroy(q)
-    est, eval_ = oracle.fifo_replay(capacity, ops, args)
+    est, eval_ = oracle.fifo_replay(model_capacity(kind, capacity), ops, args)
     assert np.array_equal(st, est)
     ok_deq = (ops == 1) & (est == 0)
     assert np.array_equal(val[ok_deq], eval_[ok_deq])
-    assert (est == oracle.ST_FULL).any() and (est == oracle.ST_EMPTY).any()
+    assert (est == oracle.ST_EMPTY).any() and (is_ymc(kind) or (est == oracle.ST_FULL).any())
 
 
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
@@ -80,6 +95,10 @@ def test_fresh_fill_full_drain(kind):
         args = [0] + list(range(1000, 1000 + n + 1)) + [0] * (n + 1)
         st, val = gq.queue_run_script(q, ops, args)
         assert st[0] == gq.GQ_EMPTY
+        if is_ymc(kind):             # no FULL: the (n+1)-th enqueue succeeds and is dequeued last
+            assert (st[1:n + 2] == gq.GQ_OK).all()
+            assert val[n + 2:2 * n + 3].tolist() == list(range(1000, 1000 + n + 1))
+            return
         assert (st[1:n + 1] == gq.GQ_OK).all() and st[n + 1] == gq.GQ_FULL
         assert val[n + 2:2 * n + 2].tolist() == list(range(1000, 1000 + n)) and st[-1] == gq.GQ_EMPTY
     finally:
@@ -97,8 +116,11 @@ def test_prefill_drain_preserves_order(kind, capacity, count):
         assert np.array_equal(out, vals)
         assert len(gq.queue_drain(q, 10)) == 0
         if count:
-            with pytest.raises(gq.GqError):            # does not fit: GQ_E_STATE
-                gq.queue_prefill(q, np.arange(capacity + 1, dtype=np.uint32))
+            if not is_ymc(kind):
+                with pytest.raises(gq.GqError):            # does not fit: GQ_E_STATE
+                    gq.queue_prefill(q, np.arange(capacity + 1, dtype=np.uint32))
+            else:
+                gq.queue_prefill(q, np.arange(7, dtype=np.uint32))
             gq.queue_reset(q)
             assert len(gq.queue_drain(q, 10)) == 0
     finally:
@@ -122,7 +144,7 @@ def test_tiny_balanced_history_is_linearizable(kind, seed):
     assert r["tot_full"] == 0 and r["tot_empty"] == 0 and len(left) == 0
     enq = recs[recs["op"] == 0]
     assert sorted(enq["arg"].tolist()) == sorted(t + i * 64 for t in range(64) for i in range(16))
-    ok, msg = oracle.check_history(to_history(recs), 128, relaxed_full=False, leftover=left)
+    ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 128), relaxed_full=False, leftover=left)
     assert ok, msg
 
 
@@ -135,19 +157,20 @@ def test_tiny_split_history_with_empty_and_full(kind, pf, seed):
         r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
                          jitter_ns=200, seed=seed, producer_fraction=pf)
         recs = gq.history_dump(q)
-        left = gq.queue_drain(q, 64)
+        left = gq.queue_drain(q, 2048)
     finally:
         gq.queue_destroy(q)
     assert len(recs) == 1024
-    assert len(left) <= 16
+    assert is_ymc(kind) or len(left) <= 16
+    assert r["pool_exhausted"] == 0
     if pf < 0.5:
         assert r["tot_empty"] > 0
     if pf > 0.5:
-        assert r["tot_full"] > 0
+        assert r["tot_full"] > 0 or is_ymc(kind)
     # exact search when it finishes; at 64-way overlap with many EMPTY/FULL returns it may not, and
     # the verdict then rests on the exact OK/EMPTY characterisation + capacity bound + conservation
-    ok, msg = oracle.check_history(to_history(recs), 16, relaxed_full=True, leftover=left, max_steps=3_000_000,
-                                   accept_unknown=True)
+    ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 16), relaxed_full=True, leftover=left,
+                                   max_steps=3_000_000, accept_unknown=True)
     assert ok, msg
 
 
@@ -161,13 +184,14 @@ def _conserve(r, left, prefill_vals=()):
 
 @pytest.mark.parametrize("kind,threads,capacity", [(k, 2048 + 32 + 5, 1 << 12) for k in KINDS] + [(k, 0, 1 << 16) for k in BIG])
 def test_balanced_fixed_ops_conserves(kind, threads, capacity):
-    q = make(kind, capacity)
+    q = make(kind, capacity, **(dict(ymc_pool_cells=1 << 26) if is_ymc(kind) else {}))
     try:
         r = gq.run_balanced(q, threads=threads, ops_per_thread=32)
-        left = gq.queue_drain(q, capacity + 1)
+        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else capacity + 1)
     finally:
         gq.queue_destroy(q)
-    assert len(left) <= capacity
+    assert is_ymc(kind) or len(left) <= capacity
+    assert r["pool_exhausted"] == 0
     assert r["tot_enq"] + r["tot_full"] == r["threads_launched"] * 32
     assert r["tot_deq"] + r["tot_empty"] == r["threads_launched"] * 32
     _conserve(r, left)
@@ -177,14 +201,15 @@ def test_balanced_fixed_ops_conserves(kind, threads, capacity):
 @pytest.mark.parametrize("kind", BIG)
 def test_balanced_timed_full_occupancy(kind):
     # BJ config 2 at full co-residency, shortened window; same launch configuration as bench.py
-    q = make(kind, 1 << 16)
+    q = make(kind, 1 << 16, **(dict(ymc_pool_cells=1 << 31) if is_ymc(kind) else {}))
     try:
         r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=20)
-        left = gq.queue_drain(q, (1 << 16) + 1)
+        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else (1 << 16) + 1)
     finally:
         gq.queue_destroy(q)
     assert r["threads_launched"] == gq.queue_max_coresident_threads(VARIANTS[kind][0], 256)
-    assert len(left) <= 1 << 16
+    assert is_ymc(kind) or len(left) <= 1 << 16
+    assert r["pool_exhausted"] == 0
     _conserve(r, left)
     assert r["succ_enq"] > 0 and r["succ_deq"] > 0
 
@@ -195,14 +220,19 @@ def test_split_timed_conserves(kind, pf):
     # BJ config 3 shape (capacity 2^20 prefilled to 50 %), shortened window
     n = 1 << 20
     pre = np.arange(n // 2, dtype=np.uint32)
-    q = make(kind, n)
+    # G-WFQ-YMC never returns FULL, so with more producers than consumers it grows for as long as
+    # it runs: fixed-op mode keeps what has to be drained (by one warp, in FIFO order) bounded
+    ymc = is_ymc(kind)
+    q = make(kind, n, **(dict(ymc_pool_cells=1 << 28) if ymc else {}))
     try:
         gq.queue_prefill(q, pre)
-        r = gq.run_split(q, threads=0, warmup_ms=2, duration_ms=10, producer_fraction=pf, seed=7, value_base=n // 2)
-        left = gq.queue_drain(q, n + 1)
+        kw = dict(ops_per_thread=40) if ymc else dict(warmup_ms=2, duration_ms=10)
+        r = gq.run_split(q, threads=0, producer_fraction=pf, seed=7, value_base=n // 2, **kw)
+        left = gq.queue_drain(q, (1 << 24) if ymc else n + 1)
     finally:
         gq.queue_destroy(q)
-    assert len(left) <= n
+    assert ymc or len(left) <= n
+    assert r["pool_exhausted"] == 0
     _conserve(r, left, pre)
     # FIFO: what is left of the prefill comes out first and in order
     pre_left = left[left < n // 2]
@@ -216,7 +246,7 @@ def test_token_protocol_at_scale(kind):
     try:
         gq.run_split(q, threads=16384, ops_per_thread=24, record_history=1, producer_fraction=0.5, seed=11)
         recs = gq.history_dump(q)
-        left = gq.queue_drain(q, (1 << 14) + 1)
+        left = gq.queue_drain(q, 1 << 18)
     finally:
         gq.queue_destroy(q)
     assert len(recs) == 16384 * 24
@@ -257,6 +287,22 @@ def test_wfq_slow_path_is_exercised_and_counts_once(kind):
         assert r["slow_enq"] + r["slow_deq"] > 0
 
 
+@pytest.mark.parametrize("kind", ["YMC-p0", "YMC-p1"])
+def test_ymc_slow_paths_are_exercised(kind):
+    # parking and the probe off, so that dequeuers really overtake enqueuers and attempts fail
+    q = make(kind, 256, max_threads=256, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
+    try:
+        r = gq.run_split(q, threads=256, block_threads=64, ops_per_thread=64, producer_fraction=0.5, seed=3)
+        left = gq.queue_drain(q, 1 << 15)
+    finally:
+        gq.queue_destroy(q)
+    assert r["pool_exhausted"] == 0
+    _conserve(r, left)
+    if kind.endswith("p0"):
+        assert r["slow_enq"] == r["tot_enq"]         # every enqueue published a request
+    assert r["slow_enq"] > 0 and r["slow_deq"] > 0
+
+
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("pf,seed", [(0.25, 1), (0.75, 2)])
 def test_tiny_split_default_parking(kind, pf, seed):
@@ -267,7 +313,7 @@ def test_tiny_split_default_parking(kind, pf, seed):
         gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
                      jitter_ns=200, seed=seed, producer_fraction=pf)
         recs = gq.history_dump(q)
-        left = gq.queue_drain(q, 64)
+        left = gq.queue_drain(q, 2048)
     finally:
         gq.queue_destroy(q)
     h = to_history(recs)
