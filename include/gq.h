@@ -56,11 +56,14 @@ typedef struct {
   uint32_t flags;           /* GQ_F_* */
   uint32_t park_ns;         /* longest wait of a dequeuer on its own vacant slot before it gives the slot up
                                (D2); default 250000 */
-  uint32_t _reserved;
+  uint32_t park_nap_ns;     /* longest single __nanosleep between two looks at a parked slot (D2); default 256 */
 } gq_opts;
 enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the warp-batched one ("naive") */
        GQ_F_NO_PROBE = 2u,      /* ablation: no read-only emptiness probe before a ticket is claimed (D1) */
-       GQ_F_NO_DEQ_SPIN = 4u    /* ablation: dequeuer invalidates a vacant slot at once, no parking (D2) */ };
+       GQ_F_NO_DEQ_SPIN = 4u,   /* ablation: dequeuer invalidates a vacant slot at once, no parking (D2) */
+       GQ_F_NO_OPT_CAS = 8u,    /* ablation: TRYENQ loads the slot before its CAS (Alg. 1 L148 as written) instead of
+                                   issuing the CAS against the predicted steady-state entry first (D3) */
+       GQ_F_COND_THR_STORE = 16u /* ablation: Threshold reset = load, compare, store (sCQ form) instead of a plain store (D4) */ };
 
 /* Device bytes queue_create_ex would need for (kind, capacity, opts). */
 size_t queue_storage_bytes(int kind, uint64_t capacity, const gq_opts* opts);

@@ -28,13 +28,15 @@ struct RingView {
   uint32_t  slot_shift; // 0 dense, 2 = 32 B, 4 = 128 B
   uint32_t  park_ns;    // D2: longest time a dequeuer waits on its own vacant slot (0 = never)
   uint32_t  park_limit; // D1: EMPTY without a ticket once Head is this far ahead of Tail
+  uint32_t  park_nap;   // D2: longest single __nanosleep between two looks at the parked slot
+  uint32_t  _pad;
 };
 
 namespace detail {
 
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
-enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u };
+enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kCondThrStore = 16u };
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
 struct LfqFmt {
@@ -58,6 +60,8 @@ struct LfqFmt {
   // <E.Cycle, 0, E.Index>
   __device__ __host__ static uint64_t unsafe(uint64_t e) { return e & ~kSafeBit; }
   __device__ __host__ static uint64_t initial() { return kSafeBit | kBot; }          // <0,1,bot> (reading G4)
+  // what the slot of a cycle-c ticket holds in steady state: the previous cycle's entry, consumed
+  __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 33) | kSafeBit | kBotC; }
 };
 
 // ---- G-WFQ entry word (Fig. 2 missing -> reading W1):
@@ -95,6 +99,8 @@ struct WfqFmt {
   __device__ __host__ static uint64_t with_note(uint64_t e, uint32_t c) { return (e & ~kNoteMask) | ((uint64_t)c << 32); }
   // Note starts "older than every cycle in use": tickets start at cycle 1, so 0 with modular compare
   __device__ __host__ static uint64_t initial() { return kSafeBit | kEnqBit | kBot; }
+  // steady state: previous cycle, consumed (CONSUME sets Enq with the index), Note never used
+  __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 48) | kSafeBit | kEnqBit | kBotC; }
 };
 
 // Hook run by a dequeuer between finding its entry and CONSUME.  G-LFQ: nothing.
@@ -118,10 +124,15 @@ struct Ring {
     return counter(w);
   }
 
-  // "reset Threshold to 3n-1" (Alg. 1): load first, store only when different, so the
-  // line stays clean in steady state (reading G8).
-  __device__ __forceinline__ static void reset_threshold(const RingView& r) {
-    if ((int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)) != r.thr_reset)
+  // "reset Threshold to 3n-1" (Alg. 1).  sCQ loads first and stores only when different, to
+  // keep the line in shared state on a cache-coherent CPU.  A GPU has no such state: every
+  // .gpu-scope access resolves at L2, so the load would only add one dependent L2 round trip to
+  // every enqueue.  Default here: a plain fire-and-forget store (the lanes of a warp name one
+  // address, so it is one L2 write per warp).  kCondThrStore restores the load-compare-store form
+  // for the ablation (reading G8).
+  __device__ __forceinline__ static void reset_threshold(const RingView& r, uint32_t flags = 0) {
+    if (!(flags & kCondThrStore) ||
+        (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)) != r.thr_reset)
       st_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)r.thr_reset);
   }
 
@@ -150,12 +161,27 @@ struct Ring {
   }
 
   // Alg. 1 L143-163.  Returns RING_OK or RING_RETRY; *t_out = the ticket used.
-  __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out) {
+  //
+  // Optimistic install (sm_100a; kNoOptCas switches it off): in steady state the slot of a
+  // cycle-c ticket holds the consumed entry of cycle c-1, <c-1, 1, bot_c>, for which every
+  // condition of L150-151 holds by construction.  The installing CAS is therefore issued
+  // against that predicted word first; when it fails, the value it returns IS the load of
+  // L148 and the listing continues from there.  One L2 round trip (FAA -> CAS) instead of two
+  // (FAA -> load -> CAS) on the common path; same linearization point (the successful CAS).
+  __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out, uint32_t flags = 0) {
     const uint64_t t = take(r.tail);                                  // L144
     *t_out = t;
     const uint32_t j = slot_of(r, t), c = cycle_of(r, t);             // L146
     uint64_t* sp = slot(r, j);
-    const uint64_t E = ld_relaxed(sp);                                // L148
+    uint64_t E;
+    if (!(flags & kNoOptCas)) {
+      E = F::predicted(c);
+      const uint64_t o = cas_release(sp, E, F::installed(E, c, x));   // L153 on the predicted entry
+      if (o == E) { reset_threshold(r, flags); return RING_OK; }      // L155
+      E = o;                                                          // L148: the failed CAS read the slot
+    } else {
+      E = ld_relaxed(sp);                                             // L148
+    }
     if (cycle_newer<F::kCycBits>(c, F::cycle(E)) && F::vacant(E)) {   // E.Cycle < c, Index in {bot,botc}
       bool ok = F::safe(E);
       if (!ok) {                                                      // (E.Safe or Head <= t), reading G5
@@ -163,7 +189,7 @@ struct Ring {
         ok = counter(ld_relaxed(r.head)) <= t;
       }
       if (ok && cas_release(sp, E, F::installed(E, c, x)) == E) {     // L153: linearization point (L111)
-        reset_threshold(r);                                           // L155
+        reset_threshold(r, flags);                                    // L155
         return RING_OK;
       }
     }
@@ -204,7 +230,7 @@ struct Ring {
     *h_out = h;
     const uint32_t j = slot_of(r, h), c = cycle_of(r, h);             // L175
     uint64_t* sp = slot(r, j);
-    uint32_t waited = 0, nap = 64;
+    uint32_t waited = 0, nap = r.park_nap < 64 ? r.park_nap : 64;
     for (;;) {
       const uint64_t E = ld_acquire(sp);                              // L176 (acquire: payload edge, G15)
       if (F::cycle(E) == c && !F::vacant(E)) {                        // L178
@@ -215,7 +241,7 @@ struct Ring {
       }
       if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
         if (waited < park_ns && F::vacant(E)) {                       // D2
-          __nanosleep(nap); waited += nap; nap = nap < 2048 ? nap * 2 : 2048;
+          __nanosleep(nap); waited += nap; nap = nap * 2 < r.park_nap ? nap * 2 : r.park_nap;
           continue;
         }
         const uint64_t New = F::vacant(E) ? F::advanced(E, c)         // L186-188

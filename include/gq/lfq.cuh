@@ -46,11 +46,11 @@ __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, u
   }
 }
 template <class F, bool kUniform, bool kWarpFaa>
-__device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, uint64_t* retries) {
+__device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, uint64_t* retries, uint32_t flags) {
   Backoff bo;
   for (;;) {
     uint64_t t;
-    if (Ring<F, kUniform, kWarpFaa>::try_enq(r, idx, &t) == RING_OK) return;
+    if (Ring<F, kUniform, kWarpFaa>::try_enq(r, idx, &t, flags) == RING_OK) return;
     ++*retries;
     bo.pause();
   }
@@ -70,7 +70,7 @@ __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32
   }
   ctx.hungry &= ~2u;
   st_relaxed32(q.data + idx, v);                                   // ordered before the release CAS below
-  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, idx, retries);
+  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, idx, retries, q.flags);
   return OK;
 }
 
@@ -85,7 +85,7 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
   }
   ctx.hungry &= ~1u;
   *out = ld_relaxed32(q.data + idx);                               // after the acquire load of the entry
-  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, idx, retries);   // release CAS: the read above is done
+  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, idx, retries, q.flags);   // release CAS: the read above is done
   return OK;
 }
 

@@ -239,11 +239,11 @@ struct Wf {
 
   // ring-level enqueue of index x: bounded fast path, then the published slow path
   template <bool kUniform, bool kWarpFaa>
-  __device__ static void ring_enq(const RingView& r, uint32_t x, uint32_t patience, uint32_t me, uint64_t* retries) {
+  __device__ static void ring_enq(const RingView& r, uint32_t x, uint32_t patience, uint32_t me, uint64_t* retries, uint32_t flags) {
     uint64_t t = 0;
     bool have_t = false;
     for (uint32_t p = 0; p < patience; ++p) {
-      if (Ring<F, kUniform, kWarpFaa>::try_enq(r, x, &t) == RING_OK) return;
+      if (Ring<F, kUniform, kWarpFaa>::try_enq(r, x, &t, flags) == RING_OK) return;
       have_t = true;
       ++*retries;
     }
@@ -342,7 +342,7 @@ __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32
   }
   ctx.hungry &= ~2u;
   st_relaxed32(q.data + idx, v);
-  Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries);
+  Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags);
   return OK;
 }
 
@@ -358,7 +358,7 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   }
   ctx.hungry &= ~1u;
   *out = ld_relaxed32(q.data + idx);
-  Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries);
+  Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, q.flags);
   return OK;
 }
 

@@ -55,7 +55,7 @@ struct YmcView {
   uint32_t nthreads;      // handle ring size k (reading Y6)
   uint32_t enq_patience, deq_patience, help_delay;
   uint32_t flags;
-  uint32_t park_ns, park_limit;
+  uint32_t park_ns, park_limit, park_nap, _pad;
 };
 
 namespace detail {
@@ -97,7 +97,7 @@ struct Ymc {
     if (i >= last(q)) { pool_exhausted(q); return kEmptyRet; }
     YmcCell* c = cell(q, i);
     uint64_t w = ld_acquire(&c->val);
-    for (uint32_t waited = 0, nap = 32; w == kBot && waited < park_ns; waited += nap, nap = nap < 1024 ? nap * 2 : 1024) {
+    for (uint32_t waited = 0, nap = 32; w == kBot && waited < park_ns; waited += nap, nap = nap * 2 < q.park_nap ? nap * 2 : q.park_nap) {
       __nanosleep(nap);                                       // D2: bounded wait on the own cell
       w = ld_acquire(&c->val);
     }

@@ -77,7 +77,7 @@ struct Layout {
   size_t off_hot = 0, off_aq = 0, off_fq = 0, off_data = 0, off_owner_aq = 0, off_owner_fq = 0, off_rec = 0, off_rec_fq = 0, off_pool = 0;
   size_t total = 0;
   uint64_t pool_cells = 0;
-  uint32_t park_ns = 0;
+  uint32_t park_ns = 0, park_nap = 0;
 };
 
 template <class Q> static int max_blocks_per_sm(int block_threads);
@@ -92,6 +92,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   if (k == 0) k = 148 * 2048;                         // no device visible: size for a full B200
   *max_threads_out = k;
   L->park_ns = o->park_ns ? o->park_ns : 250000u;
+  L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 256u;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
   if (kind == GQ_LFQ || kind == GQ_WFQ) {
@@ -159,6 +160,7 @@ static RingView make_ring(char* base, const Layout& L, size_t off_entries, size_
   r.order = L.order;
   r.slot_shift = L.slot_shift;
   r.park_ns = L.park_ns;
+  r.park_nap = L.park_nap;
   r.park_limit = (uint32_t)std::min<uint64_t>(L.N / 2, 0x7FFFFFFFu);
   return r;
 }
@@ -312,6 +314,7 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
     q->ymc.help_delay = q->opts.help_delay ? q->opts.help_delay : 1;   // [5]: after every successful dequeue
     q->ymc.flags = q->opts.flags;
     q->ymc.park_ns = L.park_ns;
+    q->ymc.park_nap = L.park_nap;
     q->ymc.park_limit = (uint32_t)std::min<uint64_t>(L.N / 2, 0x7FFFFFFFu);
   }
   rc = format_queue(q, nullptr);
