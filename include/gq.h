@@ -63,7 +63,8 @@ enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the w
        GQ_F_NO_DEQ_SPIN = 4u,   /* ablation: dequeuer invalidates a vacant slot at once, no parking (D2) */
        GQ_F_NO_OPT_CAS = 8u,    /* ablation: TRYENQ loads the slot before its CAS (Alg. 1 L148 as written) instead of
                                    issuing the CAS against the predicted steady-state entry first (D3) */
-       GQ_F_COND_THR_STORE = 16u /* ablation: Threshold reset = load, compare, store (sCQ form) instead of a plain store (D4) */ };
+       GQ_F_PLAIN_THR_STORE = 16u /* ablation: Threshold reset = plain store per enqueue instead of load-compare-store
+                                   (measured 50x slower on B200: same-address stores serialise at L2) */ };
 
 /* Device bytes queue_create_ex would need for (kind, capacity, opts). */
 size_t queue_storage_bytes(int kind, uint64_t capacity, const gq_opts* opts);

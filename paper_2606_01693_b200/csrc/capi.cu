@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <thread>
@@ -417,6 +418,11 @@ static int collect_stats(gq_queue* q, gq_run_result* res) {
 // ------------------------------------------------------------------------------- launches
 // Wait for `ev` with a host-side watchdog so that a livelocked kernel fails a call instead of
 // hanging it (SURVEY §5 "failure detection").
+static double watchdog_slack_s() {
+  const char* e = std::getenv("GQ_WATCHDOG_S");     // seconds granted on top of warmup + duration (default 60)
+  const double v = e ? std::atof(e) : 0.0;
+  return v > 0 ? v : 60.0;
+}
 static int wait_event(cudaEvent_t ev, double budget_s) {
   const auto t0 = std::chrono::steady_clock::now();
   for (;;) {
@@ -510,7 +516,7 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
   if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return le == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : cuda_fail(le, "launch"); }
   CU(cudaEventRecord(e1, nullptr));
-  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + 60.0);
+  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
   if (rc == 0) rc = finish_run(q->d_ctr, e0, e1, cfg, r, res);
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   if (rc == 0) rc = collect_stats(q, res);
@@ -544,7 +550,7 @@ static int run_ceiling(K kernel, const gq_run_cfg* cfg, gq_run_result* res, uint
   cudaError_t le = cudaLaunchCooperativeKernel((void*)kernel, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
   if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return cuda_fail(le, "launch"); }
   CU(cudaEventRecord(e1, nullptr));
-  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + 60.0);
+  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
   if (rc == 0) rc = finish_run(d_ctr, e0, e1, cfg, r, res);
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   return rc;
