@@ -36,8 +36,10 @@ template <class F, bool kUniform, bool kWarpFaa, class Fin>
 __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, uint64_t* retries, const Fin& fin,
                                              bool probe, uint32_t flags, uint64_t* ticket = nullptr) {
   Backoff bo;
+  uint32_t sn = 0;
   for (;;) {
     uint64_t h;
+    if (stuck(sn, 1, 0, ld_relaxed(r.head), ld_relaxed(r.tail))) return RING_EMPTY;
     const int s = Ring<F, kUniform, kWarpFaa>::try_deq(r, idx, &h, fin, probe, flags);
     if (s != RING_RETRY) { if (ticket) *ticket = h; return s; }
     ++*retries;
@@ -48,8 +50,10 @@ __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, u
 template <class F, bool kUniform, bool kWarpFaa>
 __device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, uint64_t* retries, uint32_t flags) {
   Backoff bo;
+  uint32_t sn = 0;
   for (;;) {
     uint64_t t;
+    if (stuck(sn, 2, 0, ld_relaxed(r.head), ld_relaxed(r.tail))) return;
     if (Ring<F, kUniform, kWarpFaa>::try_enq(r, idx, &t, flags) == RING_OK) return;
     ++*retries;
     bo.pause();

@@ -82,9 +82,12 @@ struct Wf {
                                   uint64_t target_id) {
     WfqRecord* mine = rec(r, me);
     uint64_t c = 0;
+    uint32_t sn1 = 0, sn2 = 0;
     for (;;) {
+      if (stuck(sn1, (kDeq ? 11 : 10) | ((uint32_t)((uintptr_t)r.head >> 10) & 0xF) << 8, me, ld_relaxed(G), ld_relaxed(L), ld_relaxed(kDeq ? r.tail : r.head), ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)))) return false;
       bool have = false;
       for (;;) {                                            // L249-257: FIN check, read G, help phase 2
+        if (stuck(sn2, (kDeq ? 13 : 12) | ((uint32_t)((uintptr_t)r.head >> 10) & 0xF) << 8, me, ld_relaxed(G), ld_relaxed(L), ld_relaxed(kDeq ? r.tail : r.head), ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)))) return false;
         const uint64_t lv = ld_acquire(L);
         if (tag_of(lv) != tag || (lv & kFIN)) break;
         const uint64_t g = ld_acquire(G);
@@ -147,7 +150,9 @@ struct Wf {
     using R = Ring<F, false, true>;
     const uint32_t j = R::slot_of(r, T), c = R::cycle_of(r, T);
     uint64_t* sp = R::slot(r, j);
+    uint32_t sn = 0;
     for (;;) {
+      if (stuck(sn, 20, owner, T, ld_relaxed(sp), ld_relaxed(L), v)) return true;
       const uint64_t E = ld_acquire(sp);
       if (cycle_newer<16>(c, F::cycle(E)) && cycle_newer<16>(c, F::note(E))) {
         const bool usable = F::vacant(E) && (F::safe(E) || R::counter(ld_acquire(r.head)) <= T);
@@ -184,7 +189,9 @@ struct Wf {
     using R = Ring<F, false, true>;
     const uint32_t j = R::slot_of(r, H), c = R::cycle_of(r, H);
     uint64_t* sp = R::slot(r, j);
+    uint32_t sn = 0;
     for (;;) {
+      if (stuck(sn, 21, 0, H, ld_relaxed(sp), ld_relaxed(L), v)) return true;
       uint64_t E = ld_acquire(sp);
       if (F::cycle(E) == c && F::index(E) != F::kBot)         // ready (or already consumed by the owner)
         return set_fin(L, v);
@@ -212,13 +219,19 @@ struct Wf {
 
   __device__ static void enqueue_slow(const RingView& r, uint64_t v, uint32_t x, uint32_t owner, uint32_t tag, uint32_t me) {
     uint64_t* L = &rec(r, owner)->localTail;
-    while (slow_faa<false>(r, r.tail, L, v, tag, me, (uint64_t)owner << 1))
+    uint32_t sn = 0;
+    while (slow_faa<false>(r, r.tail, L, v, tag, me, (uint64_t)owner << 1)) {
       if (try_enq_slow(r, v >> S, x, L, v, owner)) break;
+      if (stuck(sn, 30, me, ld_relaxed(r.tail), ld_relaxed(r.head), v, owner)) break;
+    }
   }
   __device__ static void dequeue_slow(const RingView& r, uint64_t v, uint32_t owner, uint32_t tag, uint32_t me) {
     uint64_t* L = &rec(r, owner)->localHead;
-    while (slow_faa<true>(r, r.head, L, v, tag, me, ((uint64_t)owner << 1) | 1))
+    uint32_t sn = 0;
+    while (slow_faa<true>(r, r.head, L, v, tag, me, ((uint64_t)owner << 1) | 1)) {
       if (try_deq_slow(r, v >> S, L, v)) break;
+      if (stuck(sn, 31, me, ld_relaxed(r.tail), ld_relaxed(r.head), v, (uint64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)))) break;
+    }
   }
 
   // Inspect one peer record ("a thread inspects one peer record every D operations");
@@ -285,6 +298,16 @@ struct Wf {
       ++*retries;
     }
     if ((int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)) < 0) return RING_EMPTY;
+    // D1 at the slow-path entry: a slow dequeue on an empty ring burns one cooperative ticket (two
+    // CAS generations on the global Head word, contended by every slow-path thread) per Threshold
+    // unit before it may report EMPTY (Alg. 2), 3N-1 of them after each successful
+    // enqueue.  The read-only observation Tail <= Head (Head read first) is the condition of
+    // Alg. 1 L197 and lets the operation linearize as EMPTY at the Tail read instead.
+    if (!(flags & kNoProbe)) {
+      const uint64_t H0 = Ring<F, kUniform, kWarpFaa>::counter(ld_acquire(r.head));
+      const uint64_t T0 = Ring<F, kUniform, kWarpFaa>::counter(ld_relaxed(r.tail));
+      if (T0 <= H0) return RING_EMPTY;
+    }
     if (!have_h) h = Ring<F, kUniform, kWarpFaa>::counter(ld_acquire(r.head)) - 1;   // seed < first ticket (see ring_enq)
     WfqRecord* my = rec(r, me);
     const uint64_t s = my->seq1;

@@ -93,7 +93,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   if (k == 0) k = 148 * 2048;                         // no device visible: size for a full B200
   *max_threads_out = k;
   L->park_ns = o->park_ns ? o->park_ns : 250000u;
-  L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 256u;
+  L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 512u;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
   if (kind == GQ_LFQ || kind == GQ_WFQ) {
@@ -479,6 +479,22 @@ static int finish_run(uint64_t* d_ctr, cudaEvent_t e0, cudaEvent_t e1, const gq_
   return 0;
 }
 
+// debug builds (-DGQ_DEBUG_STUCK=cap): report what the livelock detector recorded
+static void report_stuck() {
+#ifdef GQ_DEBUG_STUCK
+  unsigned long long h[2 + 16 * 6];
+  if (cudaMemcpyFromSymbol(h, gq::detail::g_stuck, sizeof h) != cudaSuccess) return;
+  if (!h[0]) return;
+  std::fprintf(stderr, "[gq] livelock detector fired: %llu records\n", h[1]);
+  for (unsigned i = 0; i < 16 && i < h[1]; ++i) {
+    const unsigned long long* r = h + 2 + 6 * i;
+    std::fprintf(stderr, "[gq]  loc=%#llx n=%llu tid=%llu a=%#llx b=%#llx c=%#llx d=%#llx\n", r[0] & 0xffffffffull, r[0] >> 32, r[1], r[2], r[3], r[4], r[5]);
+  }
+  std::memset(h, 0, sizeof h);
+  cudaMemcpyToSymbol(gq::detail::g_stuck, h, sizeof h);
+#endif
+}
+
 template <class Q>
 static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mode, gq_run_result* res) {
   const bool per_lane = (q->opts.flags & GQ_F_PER_LANE_FAA) != 0;
@@ -519,6 +535,7 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
   if (rc == 0) rc = finish_run(q->d_ctr, e0, e1, cfg, r, res);
   cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (rc == 0) report_stuck();
   if (rc == 0) rc = collect_stats(q, res);
   if (rc == 0 && res->pool_exhausted) return GQ_E_POOL;
   return rc;
