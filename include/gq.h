@@ -138,16 +138,37 @@ typedef struct { uint32_t proc, op, arg, ret_status, ret_val, _pad; uint64_t cal
 /* Records of the last record_history run, thread-major.  host_out: HOST. */
 int history_dump(gq_queue* q, gq_hist_rec* host_out, uint64_t max, uint64_t* n_out);
 
-/* Level-synchronous BFS with two alternating frontier queues.  d_rowptr (nv+1 uint64),
-   d_col (uint32), d_dist (nv int32, output; -1 = unreachable): DEVICE.  stats_out: HOST gq_bfs_stats. */
-typedef struct { uint32_t levels; uint32_t threads; uint64_t edges_scanned, vertices_visited, queue_ops; double ms; } gq_bfs_stats;
+/* Level-synchronous BFS with two alternating frontier queues ("At each level, the current
+   frontier is dequeued, outgoing neighbors are examined, and newly visited vertices are marked and
+   are enqueued into the next frontier.  We alternate between two queues across BFS levels until the
+   next frontier is empty").  One persistent cooperative launch; grid-wide barriers between levels.
+   d_rowptr (nv+1 uint64), d_col (uint32 ids), d_dist (nv int32, OUTPUT: hop distance, -1 =
+   unreachable): DEVICE, caller-owned.  stats_out: HOST.  The two queues (capacity pow2ceil(nv)) are
+   created and destroyed inside the call; stats.ms is the CUDA-event time of the BFS kernel alone,
+   stats.total_ms the whole call (queue creation, dist fill, kernel).  Errors: GQ_E_INVAL (src >=
+   nv, bad kind), GQ_E_POOL (G-WFQ-YMC pool exhausted), GQ_E_STATE (a frontier queue reported FULL). */
+typedef struct {
+  uint32_t threads;        /* participating threads (P:L365 sweeps 2^9..2^13); 0 = full co-residency */
+  uint32_t block_threads;  /* 0 = 256 */
+  uint32_t huge_degree;    /* adjacency lists at least this long are expanded by the whole grid; 0 = 1024 */
+  uint32_t flags;          /* GQ_F_* for the two queues */
+} gq_bfs_opts;
+typedef struct { uint32_t levels; uint32_t threads; uint64_t edges_scanned, vertices_visited, queue_ops; double ms, total_ms; } gq_bfs_stats;
 int bfs_run(int kind, const uint64_t* d_rowptr, const uint32_t* d_col, uint32_t nv, uint32_t src,
             int32_t* d_dist, gq_bfs_stats* stats_out, void* stream);
+int bfs_run_ex(int kind, const uint64_t* d_rowptr, const uint32_t* d_col, uint32_t nv, uint32_t src,
+               int32_t* d_dist, const gq_bfs_opts* opts, gq_bfs_stats* stats_out, void* stream);
 
-/* Tile-based persistent wavefront tracer with a work queue of tile ids (BASELINE.json config 5). */
+/* Tile-based persistent wavefront path tracer driven by ONE work queue of tile items ("a
+   persistent tracing kernel repeatedly dequeues work, traces rays, shades hits, and re-enqueues
+   reflective bounces ... until no work remains"; BASELINE.json config 5: "work queue of tile ids",
+   "secondary-ray batches are re-enqueued per bounce").  Item = tile | sample << 20 | bounce << 26;
+   one warp advances the 16x16 pixel-paths of an item by one bounce.  Arithmetic, camera, RNG and
+   shading constants: DESIGN.md section 6 (fp32, no FMA contraction).  d_rgb: DEVICE, height*width*3
+   floats, row-major, OUTPUT.  stats.ms = CUDA-event time of the tracing + resolve kernels. */
 typedef struct { uint32_t width, height, spp, max_bounce, n_spheres, threads; uint64_t seed;
                  const float* d_spheres; /* DEVICE, n_spheres x 8: cx,cy,cz,r, ar,ag,ab, emissive(0/1) */ } gq_rt_scene;
-typedef struct { uint64_t rays, queue_ops; double ms; } gq_rt_stats;
+typedef struct { uint64_t rays, queue_ops; double ms, total_ms; uint32_t threads, items; } gq_rt_stats;
 int rt_render(int kind, const gq_rt_scene* scene, float* d_rgb /* DEVICE H*W*3 */, gq_rt_stats* stats_out, void* stream);
 
 const char* gq_last_cuda_error(void);   /* text of the last CUDA error seen by this thread */

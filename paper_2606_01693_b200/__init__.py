@@ -57,7 +57,11 @@ class gq_run_result(C.Structure):
 
 class gq_bfs_stats(C.Structure):
     _fields_ = [("levels", C.c_uint32), ("threads", C.c_uint32), ("edges_scanned", C.c_uint64),
-                ("vertices_visited", C.c_uint64), ("queue_ops", C.c_uint64), ("ms", C.c_double)]
+                ("vertices_visited", C.c_uint64), ("queue_ops", C.c_uint64), ("ms", C.c_double), ("total_ms", C.c_double)]
+
+
+class gq_bfs_opts(C.Structure):
+    _fields_ = [("threads", C.c_uint32), ("block_threads", C.c_uint32), ("huge_degree", C.c_uint32), ("flags", C.c_uint32)]
 
 
 class gq_rt_scene(C.Structure):
@@ -66,7 +70,8 @@ class gq_rt_scene(C.Structure):
 
 
 class gq_rt_stats(C.Structure):
-    _fields_ = [("rays", C.c_uint64), ("queue_ops", C.c_uint64), ("ms", C.c_double)]
+    _fields_ = [("rays", C.c_uint64), ("queue_ops", C.c_uint64), ("ms", C.c_double), ("total_ms", C.c_double),
+                ("threads", C.c_uint32), ("items", C.c_uint32)]
 
 
 HIST_DTYPE = np.dtype([("proc", "<u4"), ("op", "<u4"), ("arg", "<u4"), ("ret_status", "<u4"), ("ret_val", "<u4"),
@@ -76,7 +81,7 @@ HIST_DTYPE = np.dtype([("proc", "<u4"), ("op", "<u4"), ("arg", "<u4"), ("ret_sta
 SYMBOLS = ("queue_storage_bytes", "queue_create", "queue_create_ex", "queue_destroy", "queue_reset", "queue_prefill",
            "queue_drain", "queue_device_view", "queue_kind", "queue_max_coresident_threads", "run_balanced",
            "run_split", "run_faa_ceiling", "run_slot_atomic_ceiling", "run_warp_faa_probe", "queue_run_script",
-           "history_dump", "bfs_run", "rt_render", "gq_last_cuda_error", "gq_version")
+           "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "gq_last_cuda_error", "gq_version")
 
 
 def _load():
@@ -102,6 +107,7 @@ def _load():
     L.queue_run_script.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
     L.history_dump.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(C.c_uint64)]
     L.bfs_run.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, P(gq_bfs_stats), C.c_void_p]
+    L.bfs_run_ex.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, P(gq_bfs_opts), P(gq_bfs_stats), C.c_void_p]
     L.rt_render.argtypes = [C.c_int, P(gq_rt_scene), C.c_void_p, P(gq_rt_stats), C.c_void_p]
     L.gq_last_cuda_error.restype = C.c_char_p
     L.gq_version.restype = C.c_char_p
@@ -225,6 +231,12 @@ def bfs_run(kind, d_rowptr, d_col, nv, src, d_dist, stream=None):
     """d_* are device pointers (ints), e.g. torch_tensor.data_ptr()."""
     st = gq_bfs_stats()
     _chk(lib.bfs_run(kind, d_rowptr, d_col, nv, src, d_dist, C.byref(st), stream), "bfs_run")
+    return {n: getattr(st, n) for n, _ in st._fields_}
+
+
+def bfs_run_ex(kind, d_rowptr, d_col, nv, src, d_dist, stream=None, **opts):
+    st = gq_bfs_stats()
+    _chk(lib.bfs_run_ex(kind, d_rowptr, d_col, nv, src, d_dist, C.byref(gq_bfs_opts(**opts)), C.byref(st), stream), "bfs_run_ex")
     return {n: getattr(st, n) for n, _ in st._fields_}
 
 

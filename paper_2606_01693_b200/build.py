@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libgq.so")
 SOURCES = [os.path.join(HERE, "csrc", f) for f in ("capi.cu", "apps.cu")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
               "-I" + os.path.join(ROOT, "include"), "-I" + os.path.join(HERE, "csrc"),
               "-shared", "-Xcompiler", "-fPIC"]
 

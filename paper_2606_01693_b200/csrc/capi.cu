@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "gq.h"
+#include "host_util.h"
 #include "kernels.cuh"
 
 using namespace gq;
@@ -20,15 +21,12 @@ using namespace gqk;
 
 // ------------------------------------------------------------------------------- errors
 static thread_local char g_err[256] = "";
-static int cuda_fail(cudaError_t e, const char* what) {
+int gq_cuda_fail(cudaError_t e, const char* what) {
   std::snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
   return e == cudaErrorMemoryAllocation ? GQ_E_NOMEM : GQ_E_CUDA;
 }
-#define CU(call)                                          \
-  do {                                                    \
-    cudaError_t e_ = (call);                              \
-    if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
-  } while (0)
+void gq_set_error(const char* text) { std::snprintf(g_err, sizeof g_err, "%s", text); }
+static int cuda_fail(cudaError_t e, const char* what) { return gq_cuda_fail(e, what); }
 
 extern "C" const char* gq_last_cuda_error(void) { return g_err; }
 extern "C" const char* gq_version(void) { return "gq 0.1 (sm_100a)"; }
@@ -57,6 +55,8 @@ struct gq_queue {
 };
 
 static int g_sms = 0;
+static int device_sms();
+int gq_device_sms() { return device_sms(); }
 static int device_sms() {
   if (!g_sms) {
     int dev = 0;
@@ -418,6 +418,10 @@ static int collect_stats(gq_queue* q, gq_run_result* res) {
 // ------------------------------------------------------------------------------- launches
 // Wait for `ev` with a host-side watchdog so that a livelocked kernel fails a call instead of
 // hanging it (SURVEY §5 "failure detection").
+static double watchdog_slack_s();
+static int wait_event(cudaEvent_t ev, double budget_s);
+double gq_watchdog_slack_s() { return watchdog_slack_s(); }
+int gq_wait_event(cudaEvent_t ev, double budget_s) { return wait_event(ev, budget_s); }
 static double watchdog_slack_s() {
   const char* e = std::getenv("GQ_WATCHDOG_S");     // seconds granted on top of warmup + duration (default 60)
   const double v = e ? std::atof(e) : 0.0;
