@@ -64,7 +64,16 @@ enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the w
        GQ_F_NO_OPT_CAS = 8u,    /* ablation: TRYENQ loads the slot before its CAS (Alg. 1 L148 as written) instead of
                                    issuing the CAS against the predicted steady-state entry first (D3) */
        GQ_F_PLAIN_THR_STORE = 16u /* ablation: Threshold reset = plain store per enqueue instead of load-compare-store
-                                   (measured 50x slower on B200: same-address stores serialise at L2) */ };
+                                   (measured 50x slower on B200: same-address stores serialise at L2) */,
+       GQ_F_THR_FIRST = 32u,    /* ablation: read and test Threshold before the Head ticket is drawn, as listed in
+                                   Alg. 1, instead of overlapping the two (D4) */
+       GQ_F_NO_PAIRED_FAA = 64u,/* ablation: G-LFQ dequeue reserves its FQ tail ticket only after the payload load has
+                                   returned, instead of behind it (D5) */
+       GQ_F_THR_RED_MAX = 128u, /* variant: Threshold reset = one red.max by the warp leader instead of load-compare-store
+                                   (measured slower on B200: it doubles the same-address atomic load) */
+       GQ_F_FENCED_PAYLOAD = 256u /* G-LFQ: order the payload against the index hand-over with release fences in front of
+                                   both installing CAS (the paper's implicit scheme) instead of the payload-cell
+                                   handshake (D6) */ };
 
 /* Device bytes queue_create_ex would need for (kind, capacity, opts). */
 size_t queue_storage_bytes(int kind, uint64_t capacity, const gq_opts* opts);

@@ -67,6 +67,9 @@ __device__ __forceinline__ uint64_t fetch_max_relaxed(uint64_t* p, uint64_t v) {
 __device__ __forceinline__ void red_max_relaxed(uint64_t* p, uint64_t v) {
   asm volatile("red.relaxed.gpu.global.max.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
 }
+__device__ __forceinline__ void red_max_s64_relaxed(int64_t* p, int64_t v) {
+  asm volatile("red.relaxed.gpu.global.max.s64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
 // CAS returning the value found (success iff result == expected).
 __device__ __forceinline__ uint64_t cas_relaxed(uint64_t* p, uint64_t expected, uint64_t desired) {
   uint64_t o; asm volatile("atom.relaxed.gpu.global.cas.b64 %0, [%1], %2, %3;" : "=l"(o) : "l"(p), "l"(expected), "l"(desired) : "memory"); return o;
@@ -107,6 +110,28 @@ __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 
   if (lane_id() == leader) base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);
   base = __shfl_sync(mask, base, leader);
   return base + (uint64_t)rank * unit;
+}
+// Two WAVEFAAs issued back to back by the same leader before either result is consumed: the two
+// L2 round trips overlap (DESIGN.md departure D5, "paired reservation").  Lemma III.1 holds for
+// each counter separately: one group, one leader, one FAA per counter, ranks from the same mask.
+template <bool kUniform>
+__device__ __forceinline__ void warp_faa2(uint64_t* ca, uint64_t* cb, uint64_t unit_a, uint64_t unit_b, uint64_t* a, uint64_t* b) {
+  uint32_t mask = __activemask();
+  if (!kUniform) {
+    const uint32_t ma = __match_any_sync(mask, reinterpret_cast<unsigned long long>(ca));
+    mask = ma & __match_any_sync(mask, reinterpret_cast<unsigned long long>(cb));
+  }
+  const uint32_t leader = __ffs(mask) - 1;
+  const uint32_t rank = __popc(mask & lanemask_lt());
+  uint64_t ba = 0, bb = 0;
+  if (lane_id() == leader) {
+    ba = faa_relaxed(ca, (uint64_t)__popc(mask) * unit_a);
+    bb = faa_relaxed(cb, (uint64_t)__popc(mask) * unit_b);
+  }
+  ba = __shfl_sync(mask, ba, leader);
+  bb = __shfl_sync(mask, bb, leader);
+  *a = ba + (uint64_t)rank * unit_a;
+  *b = bb + (uint64_t)rank * unit_b;
 }
 // The "naive" per-thread FAA of PAPER.md L95, kept for the ablation (GQ_F_PER_LANE_FAA).
 __device__ __forceinline__ uint64_t lane_faa(uint64_t* counter, uint64_t unit = 1) { return faa_relaxed(counter, unit); }

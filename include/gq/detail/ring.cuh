@@ -36,7 +36,9 @@ namespace detail {
 
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
-enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u };
+enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
+                  kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u,
+                  kRelaxedInstall = 1u << 16 /* internal: this install needs no release edge */ };
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
 struct LfqFmt {
@@ -108,6 +110,7 @@ struct NoFinalize {
   __device__ __forceinline__ void operator()(const RingView&, uint64_t /*h*/, uint32_t /*j*/, uint64_t /*E*/) const {}
 };
 
+
 template <class F, bool kUniform, bool kWarpFaa = true>
 struct Ring {
   __device__ __forceinline__ static uint64_t* slot(const RingView& r, uint32_t j) {
@@ -130,6 +133,13 @@ struct Ring {
   // B200: a plain store per enqueue (kPlainThrStore) serialises all
   // enqueuers on the Threshold word and costs 50x in throughput.
   __device__ __forceinline__ static void reset_threshold(const RingView& r, uint32_t flags = 0) {
+    if (flags & kThrRedMax) {
+      // Threshold never exceeds 3N-1, so "Threshold <- 3N-1" == max(Threshold, 3N-1): one fire-and-forget
+      // reduction by the leader of the lanes whose CAS just succeeded (all of them have their CAS result).
+      const uint32_t mask = __activemask();
+      if (lane_id() == (uint32_t)__ffs(mask) - 1) red_max_s64_relaxed(r.threshold, r.thr_reset);
+      return;
+    }
     if ((flags & kPlainThrStore) ||
         (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)) != r.thr_reset)
       st_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)r.thr_reset);
@@ -167,15 +177,18 @@ struct Ring {
   // against that predicted word first; when it fails, the value it returns IS the load of
   // L148 and the listing continues from there.  One L2 round trip (FAA -> CAS) instead of two
   // (FAA -> load -> CAS) on the common path; same linearization point (the successful CAS).
-  __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out, uint32_t flags = 0) {
-    const uint64_t t = take(r.tail);                                  // L144
+  // have/t_pre: the ticket was already reserved by the caller (D5); else it is drawn here.
+  __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out, uint32_t flags = 0,
+                                                bool have = false, uint64_t t_pre = 0) {
+    const uint64_t t = have ? t_pre : take(r.tail);                   // L144
     *t_out = t;
     const uint32_t j = slot_of(r, t), c = cycle_of(r, t);             // L146
     uint64_t* sp = slot(r, j);
     uint64_t E;
     if (!(flags & kNoOptCas)) {
       E = F::predicted(c);
-      const uint64_t o = cas_release(sp, E, F::installed(E, c, x));   // L153 on the predicted entry
+      const uint64_t o = (flags & kRelaxedInstall) ? cas_relaxed(sp, E, F::installed(E, c, x))
+                                                     : cas_release(sp, E, F::installed(E, c, x));   // L153 on the predicted entry
       if (o == E) { reset_threshold(r, flags); return RING_OK; }      // L155
       E = o;                                                          // L148: the failed CAS read the slot
     } else {
@@ -187,7 +200,8 @@ struct Ring {
         fence_acq_rel();                                              // Head must not be older than E
         ok = counter(ld_relaxed(r.head)) <= t;
       }
-      if (ok && cas_release(sp, E, F::installed(E, c, x)) == E) {     // L153: linearization point (L111)
+      if (ok && ((flags & kRelaxedInstall) ? cas_relaxed(sp, E, F::installed(E, c, x))
+                                           : cas_release(sp, E, F::installed(E, c, x))) == E) {   // L153: linearization point (L111)
         reset_threshold(r, flags);                                    // L155
         return RING_OK;
       }
@@ -214,18 +228,36 @@ struct Ring {
   //     hot Head/Tail/Threshold lines, Head does not run away from Tail, and the enqueuer
   //     that later draws ticket h hands its item straight to the parked dequeuer.  Pure delay
   //     in front of the paper's steps: every operation still finishes in bounded own steps.
+  //  D4 Threshold read overlapped with the ticket.  L166-169 ("Threshold < 0 => EMPTY") is an early
+  //     exit, not a condition the rest depends on: a dequeuer that skips it simply takes the general
+  //     path.  A caller whose last attempt on this ring succeeded (`probe` false) therefore issues
+  //     the Threshold load and the Head FAA back to back and looks at the loaded value only after
+  //     the ticket has come back: one L2 round trip instead of two.  A value below the reset value
+  //     (some dequeuer failed since the last enqueue) only matters if the slot is vacant: the D1
+  //     test is then made with the ticket in the place of Head, and parking (D2) is skipped when it
+  //     says "empty" or Threshold was negative, which leaves the listing's own steps.  kThrFirst
+  //     restores the listed order.
   template <class Finalize>
   __device__ __forceinline__ static int try_deq(const RingView& r, uint32_t* x, uint64_t* h_out, const Finalize& fin,
                                                 bool probe = false, uint32_t flags = 0) {
-    const int64_t thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
-    if (thr < 0) return RING_EMPTY;                                   // L166-169
-    const uint32_t park_ns = (flags & kNoDeqSpin) ? 0u : r.park_ns;
-    if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {       // D1
-      const uint64_t H = counter(ld_acquire(r.head));
-      const uint64_t T = counter(ld_relaxed(r.tail));
-      if (T + (park_ns ? r.park_limit : 0u) <= H) return RING_EMPTY;
+    uint32_t park_ns = (flags & kNoDeqSpin) ? 0u : r.park_ns;
+    int64_t thr;
+    uint64_t h;
+    const bool listed = probe || (flags & kThrFirst);
+    if (listed) {
+      thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
+      if (thr < 0) return RING_EMPTY;                                 // L166-169
+      if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {     // D1
+        const uint64_t H = counter(ld_acquire(r.head));
+        const uint64_t T = counter(ld_relaxed(r.tail));
+        if (T + (park_ns ? r.park_limit : 0u) <= H) return RING_EMPTY;
+      }
+      h = take(r.head);                                               // L172
+      thr = r.thr_reset;                                              // parking allowed (as before D4)
+    } else {
+      thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));   // in flight with the FAA / slot load
+      h = take(r.head);                                               // L172
     }
-    const uint64_t h = take(r.head);                                  // L172
     *h_out = h;
     const uint32_t j = slot_of(r, h), c = cycle_of(r, h);             // L175
     uint64_t* sp = slot(r, j);
@@ -240,6 +272,11 @@ struct Ring {
       }
       if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
         if (waited < park_ns && F::vacant(E)) {                       // D2
+          if (thr != r.thr_reset) {                                   // D4 path, first use of thr: some dequeuer failed since
+            const bool dead = thr < 0;                                // the last enqueue, so apply D1 now, with the ticket as Head
+            thr = r.thr_reset;
+            if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + r.park_limit <= h)) { park_ns = 0; continue; }
+          }
           __nanosleep(nap); waited += nap; nap = nap * 2 < r.park_nap ? nap * 2 : r.park_nap;
           continue;
         }

@@ -25,7 +25,7 @@ enum : int { OK = 0, FULL = 1, EMPTY = 2 };   // == GQ_OK / GQ_FULL / GQ_EMPTY o
 struct LfqView {
   RingView aq;        // allocated indices (the queue proper)
   RingView fq;        // free indices
-  uint32_t* data;     // Data[n], uint32 payloads
+  uint64_t* data;     // Data[n]: payload cells <ticket tag | v> (D6)
   uint32_t capacity;  // n
   uint32_t flags;     // GQ_F_*
 };
@@ -62,10 +62,29 @@ __device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, u
 
 }  // namespace detail
 
+// Payload cells (DESIGN.md departure D6, sm_100a).  The paper's scheme (Data[idx] <- v, then publish
+// idx) needs the payload store to be performed before the installing CAS, i.e. a release fence in
+// front of each install: MEMBAR.ALL.GPU, which waits for every outstanding store and reduction of
+// the thread and costs about two extra L2 round trips per operation on B200 (measured: 29 -> 36
+// Gops/s without them).  Instead each Data cell is one 64-bit word <tag | v>, tag = the low 32 bits
+// of the AQ tail ticket the index is installed under, and the hand-over is a handshake that needs
+// no cross-location ordering:
+//   enqueue : t <- AQ tail ticket; st Data[idx] <- <t | v>  and  CAS-install idx at slot(t), both
+//             relaxed and in flight together (a RETRY with a new ticket t' stores <t' | v> again)
+//   dequeue : h = the AQ head ticket that found idx (h == t); re-read Data[idx] until its tag is h
+// The dequeuer may arrive before the payload; the store has already been issued, so the wait is
+// bounded by memory latency, not by another thread's steps (lock-freedom is unaffected).  A tag
+// can only match the store of THIS tenure of idx: stores of earlier tenures carry tickets that
+// differ by less than 2^32 (FQ is FIFO, so an index is reused within about n + k tickets), and all
+// of them were observed by their own dequeuers, hence performed, before idx was recycled.  idx goes
+// back into FQ only after the matching load has returned its value (control dependency), so the
+// next owner's store cannot be read by it.  GQ_F_FENCED_PAYLOAD restores release CAS on both sides.
+
 // kUniform: all lanes converged at the call name the same queue (see warp_faa).
 template <bool kUniform = false, bool kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
+  using R = Ring<LfqFmt, kUniform, kWarpFaa>;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   uint32_t idx;
   if (ring_deq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, &idx, retries, NoFinalize{}, (ctx.hungry & 2u) != 0, q.flags) == RING_EMPTY) {
@@ -73,14 +92,31 @@ __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32
     return FULL;
   }
   ctx.hungry &= ~2u;
-  st_relaxed32(q.data + idx, v);                                   // ordered before the release CAS below
-  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, idx, retries, q.flags);
-  return OK;
+  uint64_t* cell = q.data + idx;
+  if (q.flags & kFencedPayload) {
+    st_relaxed(cell, v);                                           // ordered before the release CAS below
+    ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, idx, retries, q.flags);
+    return OK;
+  }
+  Backoff bo;
+  for (;;) {
+    const uint64_t t = R::take(q.aq.tail);
+    st_relaxed(cell, (t << 32) | v);                               // D6: payload tagged with its ticket
+    uint64_t tt;
+    if (R::try_enq(q.aq, idx, &tt, q.flags | kRelaxedInstall, true, t) == RING_OK) return OK;
+    ++*retries;
+    bo.pause();
+  }
 }
 
+// D5 (sm_100a): once the index is known the dequeuer will certainly enqueue it into FQ, so the
+// FQ tail ticket is reserved while the payload load is still in flight: the two L2 round trips
+// overlap.  No speculation (the ticket is always used at once) and no waiting on another thread
+// while it is held.  GQ_F_NO_PAIRED_FAA restores load-then-reserve.
 template <bool kUniform = false, bool kWarpFaa = true>
 __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32_t* out, uint64_t* retries = nullptr) {
   using namespace detail;
+  using R = Ring<LfqFmt, kUniform, kWarpFaa>;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   uint32_t idx;
   if (ring_deq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, &idx, retries, NoFinalize{}, (ctx.hungry & 1u) != 0, q.flags, &ctx.last_ticket) == RING_EMPTY) {
@@ -88,8 +124,27 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
     return EMPTY;
   }
   ctx.hungry &= ~1u;
-  *out = ld_relaxed32(q.data + idx);                               // after the acquire load of the entry
-  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, idx, retries, q.flags);   // release CAS: the read above is done
+  const bool fenced = (q.flags & kFencedPayload) != 0;
+  const uint64_t* cell = q.data + idx;
+  uint64_t w = ld_relaxed(cell);                                   // after the acquire load of the entry
+  const bool paired = !(q.flags & kNoPairedFaa);
+  uint64_t t = 0;
+  if (paired) t = R::take(q.fq.tail);                              // D5: issued behind the payload load
+  if (!fenced) {
+    const uint32_t tag = (uint32_t)ctx.last_ticket;
+    for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {   // payload still in flight
+      if (nap) __nanosleep(nap);
+      w = ld_relaxed(cell);
+    }
+  }
+  *out = (uint32_t)w;
+  const uint32_t fl = fenced ? q.flags : (q.flags | kRelaxedInstall);
+  uint64_t tt;
+  if (paired) {
+    if (R::try_enq(q.fq, idx, &tt, fl, true, t) == RING_OK) return OK;
+    ++*retries;
+  }
+  ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, idx, retries, fl);
   return OK;
 }
 

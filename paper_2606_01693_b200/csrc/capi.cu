@@ -106,7 +106,8 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
     const size_t ring_bytes = (size_t)(2 * L->N) * (8u << L->slot_shift);
     L->off_aq = off; off += ring_bytes;
     L->off_fq = off; off += ring_bytes;
-    L->off_data = off; off += align_up((size_t)capacity * 4, 256);
+    // G-LFQ: 8 B payload cells (ticket tag + value; D6); G-WFQ: plain uint32 payloads
+    L->off_data = off; off += align_up((size_t)capacity * (kind == GQ_LFQ ? 8 : 4), 256);
     if (kind == GQ_WFQ) {
       L->off_owner_aq = off; off += (size_t)(2 * L->N) * 8;
       L->off_owner_fq = off; off += (size_t)(2 * L->N) * 8;
@@ -216,6 +217,7 @@ static int format_queue(gq_queue* q, cudaStream_t st) {
   if (q->kind == GQ_LFQ) {
     format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.aq, slots, 0);
     format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.fq, slots, q->capacity);
+    CU(cudaMemsetAsync(q->lfq.data, 0, (size_t)q->capacity * 8, st));      // no payload cell carries a live ticket tag (D6)
   } else if (q->kind == GQ_WFQ) {
     format_ring_kernel<WfqFmt><<<grd, blk, 0, st>>>(q->wfq.aq, slots, 0);
     format_ring_kernel<WfqFmt><<<grd, blk, 0, st>>>(q->wfq.fq, slots, q->capacity);
@@ -287,7 +289,7 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
   if (kind == GQ_LFQ) {
     q->lfq.aq = make_ring(q->base, L, L.off_aq, 0, 0);
     q->lfq.fq = make_ring(q->base, L, L.off_fq, 0, 3);
-    q->lfq.data = reinterpret_cast<uint32_t*>(q->base + L.off_data);
+    q->lfq.data = reinterpret_cast<uint64_t*>(q->base + L.off_data);
     q->lfq.capacity = (uint32_t)capacity;
     q->lfq.flags = q->opts.flags;
   } else if (kind == GQ_WFQ) {

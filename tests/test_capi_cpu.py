@@ -37,10 +37,10 @@ def test_struct_sizes_match_header():
 def test_storage_bytes_is_pure_host_arithmetic():
     o = gq.gq_opts(max_threads=64)
     b = gq.queue_storage_bytes(gq.GQ_LFQ, 128, o)
-    # 16 KiB hot words + two rings of 2N=256 slots * 8 B + Data 128*4
-    assert b == 16 * 1024 + 2 * 256 * 8 + 512
+    # 16 KiB hot words + two rings of 2N=256 slots * 8 B + Data 128 cells * 8 B
+    assert b == 16 * 1024 + 2 * 256 * 8 + 1024
     o.layout = 2
-    assert gq.queue_storage_bytes(gq.GQ_LFQ, 128, o) == 16 * 1024 + 2 * 256 * 128 + 512
+    assert gq.queue_storage_bytes(gq.GQ_LFQ, 128, o) == 16 * 1024 + 2 * 256 * 128 + 1024
     assert gq.queue_storage_bytes(gq.GQ_LFQ, 0, o) == 0           # invalid capacity
     assert gq.queue_storage_bytes(7, 128, o) == 0                 # invalid kind
 
