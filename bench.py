@@ -37,6 +37,9 @@ CAPACITY = 1 << 16
 WARMUP_MS, DURATION_MS = 20.0, 100.0
 ALGO_BYTES_PER_OP = {"lfq": 36.5, "wfq": 37.0, "ymc": 12.0}   # SURVEY §8(d) / DESIGN.md
 KINDS = {"lfq": 0, "wfq": 1, "ymc": 2}
+# G-WFQ-YMC never reuses a cell: a 120 ms run at ~25 Gops/s touches ~1.5 G cells, so
+# the timed runs get a 2^32-cell pool (64 GiB of the 180 GB HBM); the other kinds ignore the field.
+YMC_POOL_CELLS = 1 << 32
 
 
 def env_int(name, default):
@@ -137,7 +140,7 @@ def run_ours(args, rank, world, local_rank):
     kind = KINDS[args.kind]
     full = gq.queue_max_coresident_threads(kind, 256)
     threads = args.threads or full
-    q = gq.queue_create(kind, CAPACITY)
+    q = gq.queue_create_ex(kind, CAPACITY, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     run_kw = dict(threads=threads, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns)
 
@@ -225,8 +228,9 @@ def run_ours(args, rank, world, local_rank):
         for name, k in KINDS.items():
             try:
                 fk = gq.queue_max_coresident_threads(k, 256)
-                qq = gq.queue_create(k, CAPACITY)
-            except gq.GqError:
+                qq = gq.queue_create_ex(k, CAPACITY, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
+            except gq.GqError as e:
+                sweep["balanced_" + name] = str(e)
                 continue
             pts = {}
             for th in (32, 256, 2048, 16384, 65536, fk):
@@ -236,7 +240,7 @@ def run_ours(args, rank, world, local_rank):
             gq.queue_destroy(qq)
             sweep["balanced_" + name] = pts
             try:
-                qq = gq.queue_create(k, 1 << 20)
+                qq = gq.queue_create_ex(k, 1 << 20, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
                 pre = np.arange(1 << 19, dtype=np.uint32)
                 pts = {}
                 for pf in (0.1, 0.25, 0.5, 0.75, 0.9):
