@@ -122,6 +122,20 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------ replicas
+def aggregate_replicas(dist, device, sums, maxes):
+    """Replicas only: whole-job units = SUM over ranks, time = MAX over ranks.
+    `dist` is torch.distributed (initialised) or None for a single process.  The only
+    communication of a multi-GPU run; tests/test_bench_aggregate.py drives it with gloo."""
+    import torch
+    a = torch.tensor(list(sums), dtype=torch.float64, device=device)
+    m = torch.tensor(list(maxes), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(a, op=dist.ReduceOp.SUM)
+        dist.all_reduce(m, op=dist.ReduceOp.MAX)
+    return a.tolist(), m.tolist()
+
+
 # ------------------------------------------------------------------------------ our arm
 def run_ours(args, rank, world, local_rank):
     import numpy as np
@@ -185,13 +199,8 @@ def run_ours(args, rank, world, local_rank):
     e2e_wall = time.perf_counter() - t1
 
     # ---- aggregate over ranks (replicas): ops sum, time max
-    agg = torch.tensor([ops_window, ops_all, e2e_ops], dtype=torch.float64, device="cuda")
-    tmax = torch.tensor([wall, e2e_wall, kernel_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(agg, op=dist.ReduceOp.SUM)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ops_window_all, ops_all_all, e2e_ops_all = agg.tolist()
-    wall_max, e2e_wall_max, kernel_ms_max = tmax.tolist()
+    (ops_window_all, ops_all_all, e2e_ops_all), (wall_max, e2e_wall_max, kernel_ms_max) = aggregate_replicas(
+        dist, "cuda", [ops_window, ops_all, e2e_ops], [wall, e2e_wall, kernel_ms])
 
     if rank != 0:
         if dist is not None:
@@ -209,13 +218,16 @@ def run_ours(args, rank, world, local_rank):
     peaks, peak_src = measured_peaks()
     ops_per_s_kernel = (ops_all / len(results)) / (kernel_ms * 1e-3)      # whole launch / event duration
     algo_gbps = ops_per_s_kernel * ALGO_BYTES_PER_OP[args.kind] / 1e9
-    traffic = None
+    traffic, traffic_detail = None, None
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.kind)
+        traffic_detail = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.kind)
+        traffic = traffic_detail["dram_bytes_per_launch"]      # dram__bytes_read.sum + dram__bytes_write.sum, one launch
     except Exception:
         pass
     roofline = {"bound": "l2_atomic", "achieved": ops_per_s_kernel / 1e9, "peak": 2 * c1_tps / 1e9, "unit": "Gop/s",
                 "frac": ops_per_s_kernel / (2 * c1_tps), "traffic": traffic,
+                "traffic_detail": traffic_detail, "traffic_note": "DRAM bytes of the committed ncu --set full capture of this kernel (fixed-op launch, "
+                "profiles/r1b_balanced_ncu_full.md): the rings are L2-resident, so DRAM sees the cold first touch only; L2 sector bytes per op beside it",
                 "kernel": "gqk::bench_kernel", "kernel_ms": kernel_ms,
                 "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run",
                 "c1_gtickets_s": c1_tps / 1e9, "c4_gtickets_s": c4_tps / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),

@@ -71,7 +71,14 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // ------------------------------------------------------------------------------- layout
 // One device block per queue:
 //   [ hot words, one per 1 KiB ][ AQ entries ][ FQ entries ][ Data ][ kind-specific ... ]
-static constexpr size_t kHotStride = 1024;
+// hot words (Head, Tail, Threshold of each ring) are kHotStride bytes apart; GQ_HOT_STRIDE overrides it for the
+// layout ablation (multiple of 128)
+static size_t hot_stride_init() {
+  const char* e = std::getenv("GQ_HOT_STRIDE");
+  const long v = e ? std::atol(e) : 0;
+  return (v >= 128 && v % 128 == 0 && v <= (1 << 20)) ? (size_t)v : 1024;
+}
+static const size_t kHotStride = hot_stride_init();
 struct Layout {
   uint64_t N = 0;
   uint32_t order = 0, slot_shift = 0;
