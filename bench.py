@@ -136,6 +136,70 @@ def aggregate_replicas(dist, device, sums, maxes):
     return a.tolist(), m.tolist()
 
 
+# ------------------------------------------------------------------------------ application rows
+def run_apps(gq, torch, scale, fast_oracle=True):
+    """BASELINE.json configs[3] and [4] (NEXT-1 / NEXT-2 of DESIGN.md section 6): BFS on the seeded R-MAT
+    graph and the 1920x1080 tile-queue path tracer, each checked against the oracle on the spot
+    (distances bit-exact; image within 1e-3 on >= 99.99 % of pixels) and timed beside it."""
+    import numpy as np
+    import oracle
+    from paper_2606_01693_b200 import inputs
+    out = {}
+    t0 = time.perf_counter()
+    rowptr, col, src = inputs.rmat_csr(scale, 16, seed=1)
+    gen_s = time.perf_counter() - t0
+    nv = len(rowptr) - 1
+    t0 = time.perf_counter()
+    ref, ref_edges = oracle.bfs(rowptr, col, src)
+    cpu_s = time.perf_counter() - t0
+    d_rowptr = torch.from_numpy(rowptr.view(np.int64)).cuda()
+    d_col = torch.from_numpy(col.view(np.int32)).cuda()
+    d_dist = torch.empty(nv, dtype=torch.int32, device="cuda")
+    bfs = {"graph": f"R-MAT scale {scale}, edge factor 16, {nv} vertices, {len(col)} directed edges, source {src}",
+           "generate_s": round(gen_s, 1),
+           "cpu_oracle": {"ms": round(cpu_s * 1e3, 1), "MTEPS": round(ref_edges / cpu_s / 1e6, 1), "cores": 1}}
+    for name, k in KINDS.items():
+        best = None
+        for _ in range(3):
+            st = gq.bfs_run(k, d_rowptr.data_ptr(), d_col.data_ptr(), nv, src, d_dist.data_ptr())
+            torch.cuda.synchronize()
+            if best is None or st["ms"] < best["ms"]:
+                best = st
+        exact = bool(np.array_equal(d_dist.cpu().numpy(), ref))
+        bfs[name] = {"ms": round(best["ms"], 3), "total_ms": round(best["total_ms"], 3), "levels": best["levels"],
+                     "MTEPS": round(best["edges_scanned"] / (best["ms"] * 1e-3) / 1e6, 1),
+                     "queue_Mops": round(best["queue_ops"] / (best["ms"] * 1e-3) / 1e6, 1),
+                     "threads": best["threads"], "bit_exact": exact}
+    out["bfs"] = bfs
+    del d_rowptr, d_col, d_dist
+
+    W, H, SPP, B = 1920, 1080, 4, 4
+    sph = inputs.sphere_scene(256, seed=1)
+    d_sph = torch.from_numpy(np.ascontiguousarray(sph, np.float32)).cuda()
+    d_rgb = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
+    t0 = time.perf_counter()
+    ref_img, ref_rays = oracle.rt_render(W, H, SPP, B, sph, seed=1)
+    cpu_s = time.perf_counter() - t0
+    rt = {"scene": "1920x1080, 16x16 tiles, 256 seeded spheres, 4 spp, <= 4 bounces, fp32 no FMA contraction",
+          "cpu_oracle": {"ms": round(cpu_s * 1e3, 1), "Mrays": round(ref_rays / cpu_s / 1e6, 2), "cores": oracle.hw_threads()}}
+    for name, k in KINDS.items():
+        best = None
+        for _ in range(3):
+            st = gq.rt_render(k, W, H, SPP, B, len(sph), d_sph.data_ptr(), 1, d_rgb.data_ptr())
+            torch.cuda.synchronize()
+            if best is None or st["ms"] < best["ms"]:
+                best = st
+        img = d_rgb.cpu().numpy()
+        err = np.abs(img.astype(np.float64) - ref_img.astype(np.float64)).max(axis=2)
+        rt[name] = {"ms": round(best["ms"], 3), "total_ms": round(best["total_ms"], 3),
+                    "Mrays": round(best["rays"] / (best["ms"] * 1e-3) / 1e6, 1),
+                    "queue_Mops": round(best["queue_ops"] / (best["ms"] * 1e-3) / 1e6, 3), "items": best["items"],
+                    "pixels_within_1e-3": float((err <= 1e-3).mean()), "pixels_bit_exact": float((err == 0).mean()),
+                    "rays_match_oracle": bool(best["rays"] == ref_rays)}
+    out["rt"] = rt
+    return out
+
+
 # ------------------------------------------------------------------------------ our arm
 def run_ours(args, rank, world, local_rank):
     import numpy as np
@@ -269,6 +333,10 @@ def run_ours(args, rank, world, local_rank):
             except gq.GqError as e:
                 sweep["split_" + name] = str(e)
 
+    apps = None
+    if args.apps:
+        apps = run_apps(gq, torch, args.apps_scale)
+
     # ---- CPU baseline: the oracle, as it stands, on this box's host cores (bounded sample)
     import oracle
     cores = oracle.hw_threads()
@@ -302,6 +370,8 @@ def run_ours(args, rank, world, local_rank):
         "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline, "sweep": sweep,
         "conservation": "checked every e2e step: tot_enq - tot_deq == drained",
     }
+    if apps is not None:
+        line["apps"] = apps
     print(json.dumps(line), flush=True)
     gq.queue_destroy(q)
     if dist is not None:
@@ -318,6 +388,8 @@ def main():
     ap.add_argument("--threads", type=int, default=0, help="0 = full co-residency")
     ap.add_argument("--fail-backoff-ns", type=int, default=0)
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--apps", action="store_true", help="also run BASELINE.json configs 4/5 (BFS, path tracer) against the oracle; adds minutes of host time")
+    ap.add_argument("--apps-scale", type=int, default=22, help="R-MAT scale of the BFS graph (BASELINE.json: 22)")
     args = ap.parse_args()
     rank, world, local_rank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
     if args.impl == "reference":

@@ -71,6 +71,9 @@ enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the w
                                    returned, instead of behind it (D5) */
        GQ_F_THR_RED_MAX = 128u, /* variant: Threshold reset = one red.max by the warp leader instead of load-compare-store
                                    (measured slower on B200: it doubles the same-address atomic load) */
+       GQ_F_EAGER_EMPTY = 512u, /* polling consumers (BFS, tracer): a dequeuer that sees Tail <= Head returns EMPTY at once
+                                   and parks (D2) only for an enqueuer that already holds its ticket; the default waits
+                                   in line for future enqueues, which is what the fixed-duration benchmarks want */
        GQ_F_FENCED_PAYLOAD = 256u /* G-LFQ: order the payload against the index hand-over with release fences in front of
                                    both installing CAS (the paper's implicit scheme) instead of the payload-cell
                                    handshake (D6) */ };

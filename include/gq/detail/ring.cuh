@@ -37,7 +37,7 @@ namespace detail {
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
 enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
-                  kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u,
+                  kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u, kEagerEmpty = 512u,
                   kRelaxedInstall = 1u << 16 /* internal: this install needs no release edge */ };
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
@@ -250,7 +250,7 @@ struct Ring {
       if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {     // D1
         const uint64_t H = counter(ld_acquire(r.head));
         const uint64_t T = counter(ld_relaxed(r.tail));
-        if (T + (park_ns ? r.park_limit : 0u) <= H) return RING_EMPTY;
+        if (T + ((park_ns && !(flags & kEagerEmpty)) ? r.park_limit : 0u) <= H) return RING_EMPTY;
       }
       h = take(r.head);                                               // L172
       thr = r.thr_reset;                                              // parking allowed (as before D4)
@@ -272,10 +272,14 @@ struct Ring {
       }
       if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
         if (waited < park_ns && F::vacant(E)) {                       // D2
+          if (waited == 0 && (flags & kEagerEmpty) && counter(ld_relaxed(r.tail)) <= h) {
+            park_ns = 0;                                              // polling consumers: wait only for an enqueuer that
+            continue;                                                 // already holds ticket h, never for a future one
+          }
           if (thr != r.thr_reset) {                                   // D4 path, first use of thr: some dequeuer failed since
             const bool dead = thr < 0;                                // the last enqueue, so apply D1 now, with the ticket as Head
             thr = r.thr_reset;
-            if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + r.park_limit <= h)) { park_ns = 0; continue; }
+            if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + ((flags & kEagerEmpty) ? 0u : r.park_limit) <= h)) { park_ns = 0; continue; }
           }
           __nanosleep(nap); waited += nap; nap = nap * 2 < r.park_nap ? nap * 2 : r.park_nap;
           continue;

@@ -97,6 +97,7 @@ struct Ymc {
     if (i >= last(q)) { pool_exhausted(q); return kEmptyRet; }
     YmcCell* c = cell(q, i);
     uint64_t w = ld_acquire(&c->val);
+    if (w == kBot && park_ns && (q.flags & kEagerEmpty) && ld_relaxed(q.tail) <= i) park_ns = 0;   // no enqueuer holds cell i yet
     for (uint32_t waited = 0, nap = 32; w == kBot && waited < park_ns; waited += nap, nap = nap * 2 < q.park_nap ? nap * 2 : q.park_nap) {
       __nanosleep(nap);                                       // D2: bounded wait on the own cell
       w = ld_acquire(&c->val);
@@ -183,6 +184,9 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
     if (cas_release(&Y::cell(q, i)->val, Y::kBot, val) == Y::kBot) return OK;
     id = i;
     if (retries) ++*retries;
+    // The cell was burnt by a dequeuer that found it empty, so Head has passed it: jump Tail over
+    // the whole burnt stretch at once (reading Y9) instead of drawing and failing on each cell.
+    Y::advance(q.tail, ld_acquire(q.head));
   }
   if (q.enq_patience == 0) {                                  // all-slow build: the id is a fresh, unused ticket
     id = Y::take<kUniform, kWarpFaa>(q.tail);
@@ -205,6 +209,7 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
       cas_acq_rel(&h->enq_state, Y::kPending | id, i);        // claim the request for cell i
       break;                                                  // claimed, by this CAS or by a helper's
     }
+    Y::advance(q.tail, ld_acquire(q.head));                   // reading Y9, as on the fast path
   } while (ld_acquire(&h->enq_state) & Y::kPending);
   const uint64_t cid = Y::id_of(ld_acquire(&h->enq_state));
   Y::enq_commit(q, Y::cell(q, cid), val, cid);
@@ -222,14 +227,26 @@ __device__ __forceinline__ int dequeue(const YmcView& q, thread_ctx& ctx, uint32
   if (!(q.flags & kNoProbe) && (ctx.hungry & 1u)) {           // D1: read-only emptiness probe
     const uint64_t H = ld_acquire(q.head);
     const uint64_t T = ld_relaxed(q.tail);
-    if (T + (park_ns ? q.park_limit : 0u) <= H) return EMPTY;
+    if (T + ((park_ns && !(q.flags & kEagerEmpty)) ? q.park_limit : 0u) <= H) return EMPTY;
   }
   uint64_t w = Y::kTop, id = 0;
   // fast path ([5] deq_fast)
   for (uint32_t p = 0; p < attempts; ++p) {
+    if (p > 0 && !(q.flags & kNoProbe)) {                     // D1 again before another cell is burnt: the cell just
+      const uint64_t H = ld_acquire(q.head);                  // visited was top with T beyond it (T may have been
+      const uint64_t T = ld_relaxed(q.tail);                  // caught up over burnt cells, reading Y9), which says
+      if (T <= H) { w = Y::kEmptyRet; break; }                // nothing about cells ahead; Tail <= Head does
+    }
     const uint64_t i = Y::take<kUniform, kWarpFaa>(q.head);
     w = Y::help_enq(q, ctx.tid, i, park_ns);
-    if (w == Y::kEmptyRet) break;
+    if (w == Y::kEmptyRet) {                                  // T <= i was observed: the queue is empty
+      // Catch T up to i + 1 (reading Y9; the ring's L200 "catch up Tail" carried over).  Without it every
+      // later enqueuer must draw and fail on each cell the polling dequeuers have burnt, one L2
+      // round trip per cell.  No enqueuer holds a ticket in [T, i] that it has not drawn already,
+      // and each of those cells still belongs to the dequeuer that drew it.
+      Y::advance(q.tail, i + 1);
+      break;
+    }
     if (w != Y::kTop && cas_acq_rel32(&Y::cell(q, i)->deq, Y::kBot32, Y::kTop32) == Y::kBot32) { ctx.last_ticket = i; break; }   // value claimed
     w = Y::kTop;
     id = i;
@@ -245,7 +262,7 @@ __device__ __forceinline__ int dequeue(const YmcView& q, thread_ctx& ctx, uint32
     w = i >= Y::last(q) ? Y::kTop : ld_acquire(&Y::cell(q, i)->val);
     ctx.last_ticket = i;
     Y::advance(q.head, i + 1);
-    if (w == Y::kTop) w = Y::kEmptyRet;
+    if (w == Y::kTop) { w = Y::kEmptyRet; if (i < Y::last(q)) Y::advance(q.tail, i + 1); }   // reading Y9
   }
   if (w == Y::kEmptyRet) { ctx.hungry |= 1u; return EMPTY; }
   ctx.hungry &= ~1u;
