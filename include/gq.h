@@ -56,7 +56,7 @@ typedef struct {
   uint32_t flags;           /* GQ_F_* */
   uint32_t park_ns;         /* longest wait of a dequeuer on its own vacant slot before it gives the slot up
                                (D2); default 250000 */
-  uint32_t park_nap_ns;     /* longest single __nanosleep between two looks at a parked slot (D2); default 512 */
+  uint32_t park_nap_ns;     /* longest single __nanosleep between two looks at a parked slot (D2); default 128 */
 } gq_opts;
 enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the warp-batched one ("naive") */
        GQ_F_NO_PROBE = 2u,      /* ablation: no read-only emptiness probe before a ticket is claimed (D1) */

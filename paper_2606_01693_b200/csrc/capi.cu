@@ -100,7 +100,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   if (k == 0) k = 148 * 2048;                         // no device visible: size for a full B200
   *max_threads_out = k;
   L->park_ns = o->park_ns ? o->park_ns : 250000u;
-  L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 512u;
+  L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 128u;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
   if (kind == GQ_LFQ || kind == GQ_WFQ) {

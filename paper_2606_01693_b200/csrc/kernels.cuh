@@ -35,7 +35,7 @@ __device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
 
 // One kernel for both micro-benchmarks.  kHist: record {proc,op,arg,ret,call,end} per op.
 template <class Q, bool kHist, bool kWarpFaa>
-__global__ void __launch_bounds__(512, 3) bench_kernel(Q q, BenchParams p, uint64_t* ctr, gq_hist_rec* hist) {
+__global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint64_t* ctr, gq_hist_rec* hist) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
   if (tid == 0) st_relaxed(ctr + C_T0, globaltimer_ns());

@@ -27,6 +27,12 @@ VARIANTS = {
     "G-WFQ-YMC": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22)),
     "YMC-p0": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, enq_patience=Z, deq_patience=Z)),
     "YMC-p1": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, enq_patience=1, deq_patience=1)),
+    # ablation builds: "-listed" = the paper's listing order and fences (no D3-D6),
+    # "-eager" = polling-consumer mode used by the BFS / tracer drivers
+    "G-LFQ-listed": (gq.GQ_LFQ, dict(flags=gq.GQ_F_NO_OPT_CAS | gq.GQ_F_THR_FIRST | gq.GQ_F_NO_PAIRED_FAA | gq.GQ_F_FENCED_PAYLOAD)),
+    "G-LFQ-eager": (gq.GQ_LFQ, dict(flags=gq.GQ_F_EAGER_EMPTY)),
+    "G-WFQ-eager": (gq.GQ_WFQ, dict(flags=gq.GQ_F_EAGER_EMPTY)),
+    "YMC-eager": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, flags=gq.GQ_F_EAGER_EMPTY)),
 }
 KINDS = list(VARIANTS)          # every test below runs for each of these
 SMALL = KINDS                   # tiny / single-thread cases
