@@ -15,19 +15,44 @@ from . import (GQ_LFQ, GQ_WFQ, GQ_WFQ_YMC, gq_opts, queue_create_ex, queue_destr
 KINDS = {"lfq": GQ_LFQ, "wfq": GQ_WFQ, "ymc": GQ_WFQ_YMC}
 
 
+def run_app(a):
+    """One launch of an application driver on its BASELINE.json recipe (for ncu -k regex:bfs_kernel|rt_kernel)."""
+    import torch
+    from . import bfs_run, inputs, rt_render
+    if a.mode == "bfs":
+        rowptr, col, src = inputs.rmat_csr(a.scale, 16, seed=1)
+        nv = len(rowptr) - 1
+        d_rowptr = torch.from_numpy(rowptr.view(np.int64)).cuda()
+        d_col = torch.from_numpy(col.view(np.int32)).cuda()
+        d_dist = torch.empty(nv, dtype=torch.int32, device="cuda")
+        st = bfs_run(KINDS[a.kind], d_rowptr.data_ptr(), d_col.data_ptr(), nv, src, d_dist.data_ptr())
+        torch.cuda.synchronize()
+        st["reached"] = int((d_dist >= 0).sum().item())
+    else:
+        sph = inputs.sphere_scene(256, seed=1)
+        d_sph = torch.from_numpy(np.ascontiguousarray(sph, np.float32)).cuda()
+        d_rgb = torch.empty((1080, 1920, 3), dtype=torch.float32, device="cuda")
+        st = rt_render(KINDS[a.kind], 1920, 1080, 4, 4, len(sph), d_sph.data_ptr(), 1, d_rgb.data_ptr())
+        torch.cuda.synchronize()
+    print(json.dumps({"args": vars(a), "result": st}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--kind", default="lfq", choices=list(KINDS))
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--capacity", type=int, default=1 << 16)
     ap.add_argument("--ops", type=int, default=64)
-    ap.add_argument("--mode", default="balanced", choices=["balanced", "split"])
+    ap.add_argument("--mode", default="balanced", choices=["balanced", "split", "bfs", "rt"])
+    ap.add_argument("--scale", type=int, default=20, help="bfs: R-MAT scale")
     ap.add_argument("--producer-fraction", type=float, default=0.5)
     ap.add_argument("--flags", type=int, default=0)
     ap.add_argument("--layout", type=int, default=0)
     ap.add_argument("--fail-backoff-ns", type=int, default=0)
     ap.add_argument("--pool-cells", type=int, default=0)
     a = ap.parse_args()
+    if a.mode in ("bfs", "rt"):
+        return run_app(a)
     q = queue_create_ex(KINDS[a.kind], a.capacity, gq_opts(flags=a.flags, layout=a.layout, ymc_pool_cells=a.pool_cells))
     try:
         if a.mode == "split":
