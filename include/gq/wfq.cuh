@@ -252,10 +252,17 @@ struct Wf {
 
   // ring-level enqueue of index x: bounded fast path, then the published slow path
   template <bool kUniform, bool kWarpFaa>
-  __device__ static void ring_enq(const RingView& r, uint32_t x, uint32_t patience, uint32_t me, uint64_t* retries, uint32_t flags) {
+  // have_pre/t_pre: a tail ticket the caller reserved already (D5), used by the first fast attempt
+  __device__ static void ring_enq(const RingView& r, uint32_t x, uint32_t patience, uint32_t me, uint64_t* retries, uint32_t flags,
+                                  bool have_pre = false, uint64_t t_pre = 0) {
     uint64_t t = 0;
     bool have_t = false;
-    for (uint32_t p = 0; p < patience; ++p) {
+    if (have_pre) {                                                   // consumes one unit of patience; a ticket drawn must be tried
+      if (Ring<F, kUniform, kWarpFaa>::try_enq(r, x, &t, flags, true, t_pre) == RING_OK) return;
+      have_t = true;
+      ++*retries;
+    }
+    for (uint32_t p = have_pre ? 1 : 0; p < patience; ++p) {
       if (Ring<F, kUniform, kWarpFaa>::try_enq(r, x, &t, flags) == RING_OK) return;
       have_t = true;
       ++*retries;
@@ -380,8 +387,17 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
     return EMPTY;
   }
   ctx.hungry &= ~1u;
-  *out = ld_relaxed32(q.data + idx);
-  Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, q.flags);
+  const uint32_t v = ld_relaxed32(q.data + idx);
+  // D5 as in G-LFQ: the FQ tail ticket is reserved behind the payload load (only when a fast attempt
+  // exists to use it).  D6, FQ side only: the index goes back into FQ after the payload load has
+  // delivered its value (control dependency), so the fast-path install needs no release fence;
+  // the AQ side keeps its fence (no ticket-tag handshake in G-WFQ, D6).
+  const bool paired = !(q.flags & kNoPairedFaa) && q.enq_patience != 0 && q.enq_patience != 0xFFFFFFFFu;
+  uint64_t t = 0;
+  if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq.tail);
+  *out = v;
+  const uint32_t fl = (q.flags & kFencedPayload) ? q.flags : (q.flags | kRelaxedInstall);
+  Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, fl, paired, t);
   return OK;
 }
 
