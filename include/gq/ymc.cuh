@@ -181,7 +181,9 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
   for (uint32_t p = 0; p < q.enq_patience; ++p) {
     const uint64_t i = Y::take<kUniform, kWarpFaa>(q.tail);
     if (i >= Y::last(q)) { Y::pool_exhausted(q); return FULL; }
-    if (cas_release(&Y::cell(q, i)->val, Y::kBot, val) == Y::kBot) return OK;
+    // relaxed: the word carries the payload itself and the fast path has published nothing else
+    // (the slow path's request record keeps its release/acquire discipline)
+    if (cas_relaxed(&Y::cell(q, i)->val, Y::kBot, val) == Y::kBot) return OK;
     id = i;
     if (retries) ++*retries;
     // The cell was burnt by a dequeuer that found it empty, so Head has passed it: jump Tail over
@@ -247,7 +249,8 @@ __device__ __forceinline__ int dequeue(const YmcView& q, thread_ctx& ctx, uint32
       Y::advance(q.tail, i + 1);
       break;
     }
-    if (w != Y::kTop && cas_acq_rel32(&Y::cell(q, i)->deq, Y::kBot32, Y::kTop32) == Y::kBot32) { ctx.last_ticket = i; break; }   // value claimed
+    // the claim is decided on this one word against the helpers' CAS (help_deq); the value is already in hand: relaxed
+    if (w != Y::kTop && cas_relaxed32(&Y::cell(q, i)->deq, Y::kBot32, Y::kTop32) == Y::kBot32) { ctx.last_ticket = i; break; }   // value claimed
     w = Y::kTop;
     id = i;
     if (retries) ++*retries;
