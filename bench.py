@@ -35,8 +35,8 @@ sys.path.insert(0, ROOT)
 
 CAPACITY = 1 << 16
 WARMUP_MS, DURATION_MS = 20.0, 100.0
-ALGO_BYTES_PER_OP = {"lfq": 36.5, "wfq": 37.0, "ymc": 12.0}   # SURVEY §8(d) / DESIGN.md
-KINDS = {"lfq": 0, "wfq": 1, "ymc": 2}
+ALGO_BYTES_PER_OP = {"lfq": 40.5, "wfq": 37.0, "ymc": 12.0, "lfq_direct": 12.5}   # SURVEY §8(d) / DESIGN.md section 5
+KINDS = {"lfq": 0, "wfq": 1, "ymc": 2, "lfq_direct": 3}   # lfq_direct: ablation kind (include/gq/dlfq.cuh), sweep context only
 # G-WFQ-YMC never reuses a cell: a 120 ms run at ~25 Gops/s touches ~1.5 G cells, so
 # the timed runs get a 2^32-cell pool (64 GiB of the 180 GB HBM); the other kinds ignore the field.
 YMC_POOL_CELLS = 1 << 32

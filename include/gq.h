@@ -31,7 +31,10 @@
 extern "C" {
 #endif
 
-enum { GQ_LFQ = 0, GQ_WFQ = 1, GQ_WFQ_YMC = 2 };             /* kind */
+enum { GQ_LFQ = 0, GQ_WFQ = 1, GQ_WFQ_YMC = 2,                /* kind: the paper's three queues */
+       GQ_LFQ_DIRECT = 3 };  /* ablation (not in the paper): G-LFQ without the index indirection of P:L88: one ring whose
+                                entries carry the uint32 payload; half the atomics per operation, capacity bound soft:
+                                at most capacity + (participating threads) items (include/gq/dlfq.cuh) */
 enum { GQ_OK = 0, GQ_FULL = 1, GQ_EMPTY = 2 };               /* device-op status */
 enum { GQ_E_INVAL = -1, GQ_E_NOMEM = -2, GQ_E_CUDA = -3, GQ_E_RESIDENCY = -4,
        GQ_E_TIMEOUT = -5, GQ_E_STATE = -6, GQ_E_POOL = -7 };

@@ -66,6 +66,31 @@ struct LfqFmt {
   __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 33) | kSafeBit | kBotC; }
 };
 
+// ---- direct-payload entry word (G-LFQ-D, DESIGN.md NEXT-3(i)): the uint32 payload sits where G-LFQ keeps the
+//      index, and vacancy is a bit of its own so that every 32-bit value can be stored:
+//      [63:34] Cycle(30) | [33] Safe | [32] Vacant | [31:0] payload
+struct DirFmt {
+  static constexpr int kCycBits = 30;
+  static constexpr int kCtrShift = 0;
+  static constexpr uint32_t kBotC = 0xFFFFFFFFu;
+  static constexpr uint32_t kBot = 0xFFFFFFFEu;
+  static constexpr uint64_t kIdxMask = 0xFFFFFFFFull;
+  static constexpr uint64_t kVacBit = 1ull << 32;
+  static constexpr uint64_t kSafeBit = 1ull << 33;
+  static constexpr uint64_t kConsumeMask = kVacBit | kIdxMask;       // CONSUME: Vacant <- 1, payload <- all ones
+  static constexpr uint32_t kCycMask = 0x3FFFFFFFu;
+  __device__ __host__ static uint32_t cycle(uint64_t e) { return (uint32_t)(e >> 34); }
+  __device__ __host__ static uint32_t index(uint64_t e) { return (uint32_t)e; }
+  __device__ __host__ static bool safe(uint64_t e) { return (e & kSafeBit) != 0; }
+  __device__ __host__ static bool enq_visible(uint64_t) { return true; }
+  __device__ __host__ static bool vacant(uint64_t e) { return (e & kVacBit) != 0; }
+  __device__ __host__ static uint64_t installed(uint64_t, uint32_t c, uint32_t x) { return ((uint64_t)c << 34) | kSafeBit | x; }
+  __device__ __host__ static uint64_t advanced(uint64_t e, uint32_t c) { return ((uint64_t)c << 34) | (e & kSafeBit) | kVacBit | kBot; }
+  __device__ __host__ static uint64_t unsafe(uint64_t e) { return e & ~kSafeBit; }
+  __device__ __host__ static uint64_t initial() { return kSafeBit | kVacBit | kBot; }
+  __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 34) | kSafeBit | kVacBit | kBotC; }
+};
+
 // ---- G-WFQ entry word (Fig. 2 missing -> reading W1):
 //      [63:48] Cycle(16) | [47:32] Note(16) | [31] Safe | [30] Enq | [29:0] Index(30)
 struct WfqFmt {

@@ -14,3 +14,4 @@
 #include "lfq.cuh"
 #include "wfq.cuh"
 #include "ymc.cuh"
+#include "dlfq.cuh"

@@ -136,7 +136,8 @@ def capacity_bound(h: History, capacity) -> str:
     return buf.value.decode()
 
 
-def check_history(h: History, capacity, relaxed_full=True, leftover=(), max_steps=50_000_000, accept_unknown=False):
+def check_history(h: History, capacity, relaxed_full=True, leftover=(), max_steps=50_000_000, accept_unknown=False,
+                  soft_slack=0):
     """The full pipeline of PAPER.md §IV: structural checks, token protocol (L336), the
     bad-pattern characterisation (exact for OK/EMPTY returns of the unbounded FIFO), the capacity
     lower bound, then the exact WGL search against the bounded model (L335).  Returns (ok, msg).
@@ -144,7 +145,10 @@ def check_history(h: History, capacity, relaxed_full=True, leftover=(), max_step
     accept_unknown: when the exact search runs out of budget (histories with ~64-way overlap and
     many FULL/EMPTY returns), accept on the polynomial checks alone and say so in msg.  What is
     then NOT established exactly is only the interplay of FULL returns / the capacity bound with
-    the order; FIFO order, EMPTY soundness, conservation and the capacity lower bound are."""
+    the order; FIFO order, EMPTY soundness, conservation and the capacity lower bound are.
+
+    soft_slack > 0: the direct-payload ablation queue (lincheck.hpp, relaxed_full == 2): ENQ->OK
+    legal while |S| < n + c_i, and the capacity lower bound is checked against n + soft_slack."""
     msg = precheck(h)
     if msg:
         return False, "precheck: " + msg
@@ -154,10 +158,10 @@ def check_history(h: History, capacity, relaxed_full=True, leftover=(), max_step
     r, why = poly(h)
     if r != LIN_OK:
         return False, "poly: " + why
-    msg = capacity_bound(h, capacity)
+    msg = capacity_bound(h, capacity + int(soft_slack))
     if msg:
         return False, msg
-    r, steps = wgl(h, capacity, relaxed_full, max_steps)
+    r, steps = wgl(h, capacity, 2 if soft_slack else relaxed_full, max_steps)
     if r == LIN_OK:
         return True, f"linearizable ({steps} WGL steps)"
     if r == LIN_UNKNOWN:

@@ -24,9 +24,16 @@ static std::vector<uint64_t> overlap_counts(const std::vector<Op>& h) {
 
 // One step of the model for a recorded op: is the recorded return value what the
 // sequential spec (fifo_model.hpp) would return in state m?  Applies the op if so.
-static bool model_step(FifoModel& m, const Op& o, bool relaxed_full, uint64_t ci) {
+static bool model_step(FifoModel& m, const Op& o, int relaxed_full, uint64_t ci) {
   if (o.op == OP_ENQ) {
-    if (o.status == ST_OK) return m.enq(o.arg) == ST_OK;
+    if (o.status == ST_OK) {
+      if (relaxed_full == 2) {                       // soft capacity (G-LFQ-D): |S| < n + c_i
+        if (m.s.size() >= m.capacity + ci) return false;
+        m.s.push_back(o.arg);
+        return true;
+      }
+      return m.enq(o.arg) == ST_OK;
+    }
     if (o.status == ST_FULL) {
       if (!relaxed_full) return m.s.size() >= m.capacity;
       uint64_t need = m.capacity > ci ? m.capacity - ci : 0;
@@ -77,7 +84,7 @@ std::string precheck(const std::vector<Op>& h) {
 // Definition of linearizability written out: DFS over all total orders that extend the
 // real-time partial order, replaying each prefix on the model.
 static bool brute_rec(const std::vector<Op>& h, const std::vector<uint64_t>& ci, std::vector<char>& done,
-                      size_t ndone, FifoModel& m, bool relaxed) {
+                      size_t ndone, FifoModel& m, int relaxed) {
   if (ndone == h.size()) return true;
   for (size_t i = 0; i < h.size(); ++i) {
     if (done[i]) continue;
@@ -94,7 +101,7 @@ static bool brute_rec(const std::vector<Op>& h, const std::vector<uint64_t>& ci,
   return false;
 }
 
-int brute_check(const std::vector<Op>& h, uint64_t capacity, bool relaxed_full) {
+int brute_check(const std::vector<Op>& h, uint64_t capacity, int relaxed_full) {
   if (h.size() > 12) return LIN_UNKNOWN;
   std::vector<char> done(h.size(), 0);
   FifoModel m(capacity);
@@ -112,7 +119,7 @@ struct Ev {
 };
 }  // namespace
 
-int wgl_check(const std::vector<Op>& h, uint64_t capacity, bool relaxed_full,
+int wgl_check(const std::vector<Op>& h, uint64_t capacity, int relaxed_full,
               uint64_t max_steps, uint64_t* steps_out) {
   const size_t m = h.size();
   if (steps_out) *steps_out = 0;

@@ -24,6 +24,10 @@
 // no-op when |S| >= n - c_i, c_i = number of other operations whose interval overlaps
 // operation i (they may each hold one index of the indirection layer).
 // Without it FULL is strict (|S| == n).  EMPTY is always strict.
+// relaxed_full == 2 (the direct-payload ablation queue G-LFQ-D, which is not in the paper): the
+// capacity is soft on both sides: ENQ->OK is legal while |S| < n + c_i (an enqueue that passed its
+// "Tail - Head < n" test at t0 installs at t1 after at most c_i other enqueues linearized in
+// between, all of which overlap it), ENQ->FULL as above.
 #pragma once
 #include <cstdint>
 #include <string>
@@ -43,8 +47,8 @@ enum Verdict : int { LIN_OK = 1, LIN_VIOLATION = 0, LIN_UNKNOWN = -1, LIN_MALFOR
 // OK-enqueued values unique (required by poly_check and by the token protocol, L336).
 std::string precheck(const std::vector<Op>& h);
 
-int brute_check(const std::vector<Op>& h, uint64_t capacity, bool relaxed_full);
-int wgl_check(const std::vector<Op>& h, uint64_t capacity, bool relaxed_full,
+int brute_check(const std::vector<Op>& h, uint64_t capacity, int relaxed_full);
+int wgl_check(const std::vector<Op>& h, uint64_t capacity, int relaxed_full,
               uint64_t max_steps, uint64_t* steps_out);
 // returns LIN_VIOLATION with a reason, or LIN_OK meaning "no bad pattern found".
 int poly_check(const std::vector<Op>& h, std::string* why);

@@ -45,13 +45,13 @@ int orc_precheck(uint64_t m, const uint32_t* proc, const uint32_t* op, const uin
 
 int orc_brute(uint64_t m, const uint32_t* proc, const uint32_t* op, const uint32_t* arg, const uint32_t* status,
               const uint32_t* val, const uint64_t* call, const uint64_t* end, uint64_t capacity, int relaxed_full) {
-  return brute_check(gather(m, proc, op, arg, status, val, call, end), capacity, relaxed_full != 0);
+  return brute_check(gather(m, proc, op, arg, status, val, call, end), capacity, relaxed_full);
 }
 
 int orc_wgl(uint64_t m, const uint32_t* proc, const uint32_t* op, const uint32_t* arg, const uint32_t* status,
             const uint32_t* val, const uint64_t* call, const uint64_t* end, uint64_t capacity, int relaxed_full,
             uint64_t max_steps, uint64_t* steps_out) {
-  return wgl_check(gather(m, proc, op, arg, status, val, call, end), capacity, relaxed_full != 0, max_steps, steps_out);
+  return wgl_check(gather(m, proc, op, arg, status, val, call, end), capacity, relaxed_full, max_steps, steps_out);
 }
 
 int orc_poly(uint64_t m, const uint32_t* proc, const uint32_t* op, const uint32_t* arg, const uint32_t* status,

@@ -12,7 +12,7 @@ import numpy as np
 
 from .build import LIB, build as _build
 
-GQ_LFQ, GQ_WFQ, GQ_WFQ_YMC = 0, 1, 2
+GQ_LFQ, GQ_WFQ, GQ_WFQ_YMC, GQ_LFQ_DIRECT = 0, 1, 2, 3
 GQ_OK, GQ_FULL, GQ_EMPTY = 0, 1, 2
 GQ_OP_ENQ, GQ_OP_DEQ = 0, 1
 GQ_E_INVAL, GQ_E_NOMEM, GQ_E_CUDA, GQ_E_RESIDENCY, GQ_E_TIMEOUT, GQ_E_STATE, GQ_E_POOL = -1, -2, -3, -4, -5, -6, -7

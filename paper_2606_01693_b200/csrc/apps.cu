@@ -29,14 +29,17 @@ __device__ __forceinline__ uint64_t warp_sum64(uint64_t v) {
 // G-WFQ-YMC after EMPTY dequeues has H > T with the cells in between burnt: move T up to H before
 // the queue is filled again (what the failed tickets would do one by one).
 __device__ __forceinline__ void requeue_prepare(const LfqView&) {}
+__device__ __forceinline__ void requeue_prepare(const DlfqView&) {}
 __device__ __forceinline__ void requeue_prepare(const WfqView&) {}
 __device__ __forceinline__ void requeue_prepare(const YmcView& q) { Ymc::advance(q.tail, ld_acquire(q.head)); }
 __device__ __forceinline__ bool pool_exhausted(const LfqView&) { return false; }
+__device__ __forceinline__ bool pool_exhausted(const DlfqView&) { return false; }
 __device__ __forceinline__ bool pool_exhausted(const WfqView&) { return false; }
 __device__ __forceinline__ bool pool_exhausted(const YmcView& q) { return ld_relaxed(q.exhausted) != 0; }
 
 template <class Q> struct ViewOf;
 template <> struct ViewOf<LfqView> { static constexpr int kind = GQ_LFQ; };
+template <> struct ViewOf<DlfqView> { static constexpr int kind = GQ_LFQ_DIRECT; };
 template <> struct ViewOf<WfqView> { static constexpr int kind = GQ_WFQ; };
 template <> struct ViewOf<YmcView> { static constexpr int kind = GQ_WFQ_YMC; };
 
@@ -264,6 +267,7 @@ extern "C" int bfs_run_ex(int kind, const uint64_t* d_rowptr, const uint32_t* d_
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   switch (kind) {
     case GQ_LFQ: return bfs_run_t<LfqView>(d_rowptr, d_col, nv, src, d_dist, o, stats_out, st);
+    case GQ_LFQ_DIRECT: return bfs_run_t<DlfqView>(d_rowptr, d_col, nv, src, d_dist, o, stats_out, st);
     case GQ_WFQ: return bfs_run_t<WfqView>(d_rowptr, d_col, nv, src, d_dist, o, stats_out, st);
     case GQ_WFQ_YMC: return bfs_run_t<YmcView>(d_rowptr, d_col, nv, src, d_dist, o, stats_out, st);
     default: return GQ_E_INVAL;
@@ -578,6 +582,7 @@ extern "C" int rt_render(int kind, const gq_rt_scene* scene, float* d_rgb, gq_rt
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   switch (kind) {
     case GQ_LFQ: return rt_render_t<LfqView>(*scene, d_rgb, stats_out, st);
+    case GQ_LFQ_DIRECT: return rt_render_t<DlfqView>(*scene, d_rgb, stats_out, st);
     case GQ_WFQ: return rt_render_t<WfqView>(*scene, d_rgb, stats_out, st);
     case GQ_WFQ_YMC: return rt_render_t<YmcView>(*scene, d_rgb, stats_out, st);
     default: return GQ_E_INVAL;

@@ -45,6 +45,7 @@ struct gq_queue {
   size_t bytes = 0;
   bool owns = false;
   LfqView lfq{};
+  DlfqView dlfq{};
   WfqView wfq{};
   YmcView ymc{};
   uint64_t* d_ctr = nullptr;        // C_COUNT result counters
@@ -93,7 +94,7 @@ template <class Q> static int max_blocks_per_sm(int block_threads);
 static uint32_t default_max_threads(int kind);
 
 static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout* L, uint32_t* max_threads_out) {
-  if (kind < GQ_LFQ || kind > GQ_WFQ_YMC || capacity < 1) return GQ_E_INVAL;
+  if (kind < GQ_LFQ || kind > GQ_LFQ_DIRECT || capacity < 1) return GQ_E_INVAL;
   gq_opts z{}; if (!o) o = &z;
   if (o->layout > 2) return GQ_E_INVAL;
   uint32_t k = o->max_threads ? o->max_threads : default_max_threads(kind);
@@ -103,7 +104,13 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 128u;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
-  if (kind == GQ_LFQ || kind == GQ_WFQ) {
+  if (kind == GQ_LFQ_DIRECT) {                        // one ring, payload in the entry word: no FQ, no Data
+    if (capacity >= (1ull << 31)) return GQ_E_INVAL;
+    L->N = pow2ceil(std::max<uint64_t>(capacity, k));
+    L->order = 0; while ((1ull << L->order) < 2 * L->N) ++L->order;
+    L->slot_shift = o->layout == 0 ? 0 : (o->layout == 1 ? 2 : 4);
+    L->off_aq = off; off += (size_t)(2 * L->N) * (8u << L->slot_shift);
+  } else if (kind == GQ_LFQ || kind == GQ_WFQ) {
     const uint64_t idx_limit = kind == GQ_LFQ ? 0xFFFFFFFEull : 0x3FFFFFFEull;
     if (capacity >= idx_limit) return GQ_E_INVAL;
     if (kind == GQ_WFQ && k >= WfqFmt::kThrNull) return GQ_E_INVAL;
@@ -221,7 +228,9 @@ static int format_queue(gq_queue* q, cudaStream_t st) {
   }
   const uint64_t slots = 2 * q->N;
   const unsigned blk = 256, grd = (unsigned)((slots + blk - 1) / blk);
-  if (q->kind == GQ_LFQ) {
+  if (q->kind == GQ_LFQ_DIRECT) {
+    format_ring_kernel<DirFmt><<<grd, blk, 0, st>>>(q->dlfq.r, slots, 0);
+  } else if (q->kind == GQ_LFQ) {
     format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.aq, slots, 0);
     format_ring_kernel<LfqFmt><<<grd, blk, 0, st>>>(q->lfq.fq, slots, q->capacity);
     CU(cudaMemsetAsync(q->lfq.data, 0, (size_t)q->capacity * 8, st));      // no payload cell carries a live ticket tag (D6)
@@ -250,6 +259,7 @@ static int kind_blocks_per_sm(int kind, int block_threads) {
     case GQ_LFQ: return max_blocks_per_sm<LfqView>(block_threads);
     case GQ_WFQ: return max_blocks_per_sm<WfqView>(block_threads);
     case GQ_WFQ_YMC: return max_blocks_per_sm<YmcView>(block_threads);
+    case GQ_LFQ_DIRECT: return max_blocks_per_sm<DlfqView>(block_threads);
     default: return 0;
   }
 }
@@ -260,7 +270,7 @@ static uint32_t default_max_threads(int kind) {
 }
 
 extern "C" int queue_max_coresident_threads(int kind, int block_threads, uint32_t* out) {
-  if (!out || kind < GQ_LFQ || kind > GQ_WFQ_YMC) return GQ_E_INVAL;
+  if (!out || kind < GQ_LFQ || kind > GQ_LFQ_DIRECT) return GQ_E_INVAL;
   if (block_threads <= 0) block_threads = 256;
   if (block_threads % 32 || block_threads > 512) return GQ_E_INVAL;
   const int sms = device_sms();
@@ -293,7 +303,11 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
   }
   cudaError_t e = cudaMalloc(&q->d_ctr, C_COUNT * sizeof(uint64_t));
   if (e != cudaSuccess) { if (q->owns) cudaFree(q->base); delete q; return cuda_fail(e, "cudaMalloc(counters)"); }
-  if (kind == GQ_LFQ) {
+  if (kind == GQ_LFQ_DIRECT) {
+    q->dlfq.r = make_ring(q->base, L, L.off_aq, 0, 0);
+    q->dlfq.capacity = (uint32_t)capacity;
+    q->dlfq.flags = q->opts.flags;
+  } else if (kind == GQ_LFQ) {
     q->lfq.aq = make_ring(q->base, L, L.off_aq, 0, 0);
     q->lfq.fq = make_ring(q->base, L, L.off_fq, 0, 3);
     q->lfq.data = reinterpret_cast<uint64_t*>(q->base + L.off_data);
@@ -362,6 +376,7 @@ extern "C" int queue_device_view(const gq_queue* q, void* view_out, size_t view_
   const void* src = nullptr; size_t n = 0;
   switch (q->kind) {
     case GQ_LFQ: src = &q->lfq; n = sizeof(LfqView); break;
+    case GQ_LFQ_DIRECT: src = &q->dlfq; n = sizeof(DlfqView); break;
     case GQ_WFQ: src = &q->wfq; n = sizeof(WfqView); break;
     default: src = &q->ymc; n = sizeof(YmcView); break;
   }
@@ -377,10 +392,12 @@ static int dispatch(gq_queue* q, Fn&& fn) {
     case GQ_LFQ: return fn(q->lfq);
     case GQ_WFQ: return fn(q->wfq);
     case GQ_WFQ_YMC: return fn(q->ymc);
+    case GQ_LFQ_DIRECT: return fn(q->dlfq);
     default: return GQ_E_INVAL;
   }
 }
 static void set_nthreads(LfqView&, uint32_t) {}
+static void set_nthreads(DlfqView&, uint32_t) {}
 static void set_nthreads(WfqView& v, uint32_t n) { v.nthreads = n; }
 static void set_nthreads(YmcView& v, uint32_t n) { v.nthreads = n; }
 
@@ -407,7 +424,7 @@ __global__ void ymc_stats_kernel(YmcHandle* a, uint32_t n, uint64_t* out) {
   if ((threadIdx.x & 31) == 0) { if (se) red_add_relaxed(out, se); if (sd) red_add_relaxed(out + 1, sd); if (hp) red_add_relaxed(out + 2, hp); }
 }
 static int collect_stats(gq_queue* q, gq_run_result* res) {
-  if (q->kind == GQ_LFQ) return 0;
+  if (q->kind == GQ_LFQ || q->kind == GQ_LFQ_DIRECT) return 0;
   uint64_t* d = nullptr; uint64_t h[4] = {0, 0, 0, 0};
   CU(cudaMalloc(&d, 32)); cudaMemset(d, 0, 32);
   if (q->kind == GQ_WFQ)
@@ -654,7 +671,7 @@ extern "C" int queue_prefill(gq_queue* q, const uint32_t* host_vals, uint64_t co
   // Lanes enqueue side by side only where ticket order is certain to be lane order: a freshly
   // formatted queue on its fast path.  Anywhere else (holes left by abandoned tickets after a
   // concurrent run, all-slow builds) the lanes take turns.
-  const uint32_t serial = !q->fresh || (q->kind != GQ_LFQ && q->opts.enq_patience == GQ_PATIENCE_ZERO);
+  const uint32_t serial = !q->fresh || (q->kind != GQ_LFQ && q->kind != GQ_LFQ_DIRECT && q->opts.enq_patience == GQ_PATIENCE_ZERO);
   q->fresh = false;
   return dispatch(q, [&](auto& view) { return prefill_t(view, host_vals, count, st, serial); });
 }

@@ -119,6 +119,7 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
 //  - all-slow builds (patience 0) place concurrent requests in any order, which is linearizable
 //    but not array order: `serial` makes the lanes take turns.
 __device__ __forceinline__ void prefill_prepare(const LfqView&) {}
+__device__ __forceinline__ void prefill_prepare(const DlfqView&) {}
 __device__ __forceinline__ void prefill_prepare(const WfqView&) {}
 __device__ __forceinline__ void prefill_prepare(const YmcView& q) { Ymc::advance(q.tail, ld_acquire(q.head)); }
 

@@ -11,8 +11,8 @@ from paper_2606_01693_b200 import inputs
 pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
-KINDS = [gq.GQ_LFQ, gq.GQ_WFQ, gq.GQ_WFQ_YMC]
-IDS = ["G-LFQ", "G-WFQ", "G-WFQ-YMC"]
+KINDS = [gq.GQ_LFQ, gq.GQ_WFQ, gq.GQ_WFQ_YMC, gq.GQ_LFQ_DIRECT]
+IDS = ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-D"]
 
 
 def run_bfs(kind, rowptr, col, src, **opts):

@@ -260,3 +260,17 @@ def test_capacity_lower_bound():
     # a dequeue invoked before the third enqueue finished may have made room
     rows2 = rows + [(3, D, 0, 0, 1, 3, 5)]
     assert oracle.capacity_bound(H(rows2), 2) == ""
+
+
+def test_soft_capacity_mode_for_the_direct_payload_ablation():
+    # relaxed_full == 2 (lincheck.hpp): ENQ->OK legal while |S| < n + c_i.  n = 1:
+    # two overlapping enqueues may both succeed (each has c_i = 1) ...
+    rows = [(0, E, 7, 0, 0, 0, 10), (1, E, 8, 0, 0, 1, 9), (0, D, 0, 0, 8, 20, 21), (0, D, 0, 0, 7, 22, 23)]
+    assert oracle.brute(H(rows), 1, 2) == LIN_OK and oracle.wgl(H(rows), 1, 2)[0] == LIN_OK
+    assert oracle.brute(H(rows), 1, 1) == LIN_VIOLATION            # the paper's bound: |S| <= n always
+    # ... but two enqueues ordered in real time may not (the second has c_i = 0)
+    rows = [(0, E, 7, 0, 0, 0, 1), (1, E, 8, 0, 0, 2, 3), (0, D, 0, 0, 7, 20, 21), (0, D, 0, 0, 8, 22, 23)]
+    assert oracle.brute(H(rows), 1, 2) == LIN_VIOLATION and oracle.wgl(H(rows), 1, 2)[0] == LIN_VIOLATION
+    # FIFO order is untouched by the soft bound
+    rows = [(0, E, 7, 0, 0, 0, 1), (1, E, 8, 0, 0, 2, 3), (0, D, 0, 0, 8, 20, 21)]
+    assert oracle.brute(H(rows), 4, 2) == LIN_VIOLATION

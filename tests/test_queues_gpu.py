@@ -33,16 +33,28 @@ VARIANTS = {
     "G-LFQ-eager": (gq.GQ_LFQ, dict(flags=gq.GQ_F_EAGER_EMPTY)),
     "G-WFQ-eager": (gq.GQ_WFQ, dict(flags=gq.GQ_F_EAGER_EMPTY)),
     "YMC-eager": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, flags=gq.GQ_F_EAGER_EMPTY)),
+    # direct-payload single-ring ablation (include/gq/dlfq.cuh): capacity bound soft, at most n + k items
+    "G-LFQ-D": (gq.GQ_LFQ_DIRECT, {}),
+    "G-LFQ-D-eager": (gq.GQ_LFQ_DIRECT, dict(flags=gq.GQ_F_EAGER_EMPTY)),
 }
 KINDS = list(VARIANTS)          # every test below runs for each of these
 SMALL = KINDS                   # tiny / single-thread cases
-BIG = ["G-LFQ", "G-WFQ", "G-WFQ-YMC"]        # full-occupancy cases
+BIG = ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-D"]        # full-occupancy cases
 IDS = KINDS
 UNBOUNDED = 1 << 31
 
 
 def is_ymc(kind):
     return VARIANTS[kind][0] == gq.GQ_WFQ_YMC
+
+
+def is_direct(kind):
+    return VARIANTS[kind][0] == gq.GQ_LFQ_DIRECT
+
+
+def soft_slack(kind, threads):
+    """G-LFQ-D may hold up to n + k items for a moment (dlfq.cuh); every other kind is exact."""
+    return threads if is_direct(kind) else 0
 
 
 def model_capacity(kind, capacity):
@@ -167,7 +179,7 @@ def test_tiny_split_history_with_empty_and_full(kind, pf, seed):
     finally:
         gq.queue_destroy(q)
     assert len(recs) == 1024
-    assert is_ymc(kind) or len(left) <= 16
+    assert is_ymc(kind) or len(left) <= 16 + soft_slack(kind, 64)
     assert r["pool_exhausted"] == 0
     if pf < 0.5:
         assert r["tot_empty"] > 0
@@ -176,7 +188,7 @@ def test_tiny_split_history_with_empty_and_full(kind, pf, seed):
     # exact search when it finishes; at 64-way overlap with many EMPTY/FULL returns it may not, and
     # the verdict then rests on the exact OK/EMPTY characterisation + capacity bound + conservation
     ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 16), relaxed_full=True, leftover=left,
-                                   max_steps=3_000_000, accept_unknown=True)
+                                   max_steps=3_000_000, accept_unknown=True, soft_slack=soft_slack(kind, 64))
     assert ok, msg
 
 
@@ -193,10 +205,10 @@ def test_balanced_fixed_ops_conserves(kind, threads, capacity):
     q = make(kind, capacity, **(dict(ymc_pool_cells=1 << 26) if is_ymc(kind) else {}))
     try:
         r = gq.run_balanced(q, threads=threads, ops_per_thread=32)
-        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else capacity + 1)
+        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else capacity + 1 + soft_slack(kind, 1 << 18))
     finally:
         gq.queue_destroy(q)
-    assert is_ymc(kind) or len(left) <= capacity
+    assert is_ymc(kind) or len(left) <= capacity + soft_slack(kind, r["threads_launched"])
     assert r["pool_exhausted"] == 0
     assert r["tot_enq"] + r["tot_full"] == r["threads_launched"] * 32
     assert r["tot_deq"] + r["tot_empty"] == r["threads_launched"] * 32
@@ -210,11 +222,11 @@ def test_balanced_timed_full_occupancy(kind):
     q = make(kind, 1 << 16, **(dict(ymc_pool_cells=1 << 31) if is_ymc(kind) else {}))
     try:
         r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=20)
-        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else (1 << 16) + 1)
+        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else (1 << 16) + 1 + soft_slack(kind, 1 << 18))
     finally:
         gq.queue_destroy(q)
     assert r["threads_launched"] == gq.queue_max_coresident_threads(VARIANTS[kind][0], 256)
-    assert is_ymc(kind) or len(left) <= 1 << 16
+    assert is_ymc(kind) or len(left) <= (1 << 16) + soft_slack(kind, r["threads_launched"])
     assert r["pool_exhausted"] == 0
     _conserve(r, left)
     assert r["succ_enq"] > 0 and r["succ_deq"] > 0
@@ -234,10 +246,10 @@ def test_split_timed_conserves(kind, pf):
         gq.queue_prefill(q, pre)
         kw = dict(ops_per_thread=40) if ymc else dict(warmup_ms=2, duration_ms=10)
         r = gq.run_split(q, threads=0, producer_fraction=pf, seed=7, value_base=n // 2, **kw)
-        left = gq.queue_drain(q, (1 << 24) if ymc else n + 1)
+        left = gq.queue_drain(q, (1 << 24) if ymc else n + 1 + soft_slack(kind, 1 << 18))
     finally:
         gq.queue_destroy(q)
-    assert ymc or len(left) <= n
+    assert ymc or len(left) <= n + soft_slack(kind, r["threads_launched"])
     assert r["pool_exhausted"] == 0
     _conserve(r, left, pre)
     # FIFO: what is left of the prefill comes out first and in order
