@@ -9,10 +9,10 @@ import json
 
 import numpy as np
 
-from . import (GQ_LFQ, GQ_WFQ, GQ_WFQ_YMC, gq_opts, queue_create_ex, queue_destroy, queue_drain, queue_prefill,
+from . import (GQ_LFQ, GQ_LFQ_DIRECT, GQ_WFQ, GQ_WFQ_YMC, gq_opts, queue_create_ex, queue_destroy, queue_drain, queue_prefill,
                run_balanced, run_split)
 
-KINDS = {"lfq": GQ_LFQ, "wfq": GQ_WFQ, "ymc": GQ_WFQ_YMC}
+KINDS = {"lfq": GQ_LFQ, "wfq": GQ_WFQ, "ymc": GQ_WFQ_YMC, "lfq_direct": GQ_LFQ_DIRECT}
 
 
 def run_app(a):

@@ -338,3 +338,19 @@ def test_tiny_split_default_parking(kind, pf, seed):
     assert oracle.precheck(h) == "" and oracle.conservation(h, left) == ""
     r, why = oracle.poly(h)
     assert r == oracle.LIN_OK, why
+
+
+# ---------------------------------------------------------------- soak: past every 32-bit wrap
+@pytest.mark.parametrize("kind", ["G-LFQ", "G-WFQ"])
+def test_soak_past_the_ticket_tag_wrap(kind):
+    # G-LFQ's payload cells carry the low 32 bits of the AQ ticket (D6) and payload values are
+    # tid + iter*k mod 2^32: 600 ms at full co-residency is ~2.5e10 operations, i.e. more than 2^32 tickets
+    # on each ring and more than 2^32 enqueues; G-WFQ's 16-bit cycle field wraps every 2^35 tickets.
+    q = make(kind, 1 << 16)
+    try:
+        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=600)
+        left = gq.queue_drain(q, (1 << 16) + 1)
+    finally:
+        gq.queue_destroy(q)
+    assert r["tot_enq"] + r["tot_deq"] > (1 << 33)
+    _conserve(r, left)
