@@ -37,7 +37,7 @@ static_assert(sizeof(WfqRecord) == 128, "one L2 line per record");
 
 struct WfqView {
   RingView aq, fq;          // RingView::rec -> WfqRecord[nthreads] of that ring, ::owner -> Owner[2N]
-  uint32_t* data;
+  uint64_t* data;           // Data[n]: payload cells <ticket tag | v> (D6; the tag is used for fast-path installs only)
   uint32_t capacity;
   uint32_t nthreads;        // help ring size k (reading W7)
   uint32_t enq_patience, deq_patience, help_delay;
@@ -45,6 +45,13 @@ struct WfqView {
 };
 
 namespace detail {
+
+// D6 in G-WFQ.  A fast-path enqueue knows its AQ ticket before it installs, so it can use G-LFQ's
+// ticket-tagged payload cell and a relaxed install; a slow-path install happens at a ticket the owner
+// does not know in advance (a helper may do it), so it keeps the release/acquire chain of the request
+// record instead.  The dequeuer must know which kind of entry it consumed: fast-path installs set
+// bit 29 of the 30-bit Index field (indices are < 2^29 - 2), slow-path installs leave it clear.
+constexpr uint32_t kWfqFast = 1u << 29, kWfqIdxMask = kWfqFast - 1u;
 
 struct Wf {
   using F = WfqFmt;
@@ -251,22 +258,30 @@ struct Wf {
   }
 
   // ring-level enqueue of index x: bounded fast path, then the published slow path
+  // have_pre/t_pre: a tail ticket the caller reserved already (D5), used by the first fast attempt.
+  // cell/v (AQ side with D6): every fast attempt stores <its ticket | v> into the payload cell and
+  // installs x | kWfqFast with a relaxed CAS; the slow path installs plain x behind the record's fences.
   template <bool kUniform, bool kWarpFaa>
-  // have_pre/t_pre: a tail ticket the caller reserved already (D5), used by the first fast attempt
   __device__ static void ring_enq(const RingView& r, uint32_t x, uint32_t patience, uint32_t me, uint64_t* retries, uint32_t flags,
-                                  bool have_pre = false, uint64_t t_pre = 0) {
+                                  bool have_pre = false, uint64_t t_pre = 0, uint64_t* cell = nullptr, uint32_t v = 0) {
+    using R = Ring<F, kUniform, kWarpFaa>;
     uint64_t t = 0;
     bool have_t = false;
     if (have_pre) {                                                   // consumes one unit of patience; a ticket drawn must be tried
-      if (Ring<F, kUniform, kWarpFaa>::try_enq(r, x, &t, flags, true, t_pre) == RING_OK) return;
+      if (R::try_enq(r, x, &t, flags, true, t_pre) == RING_OK) return;
       have_t = true;
       ++*retries;
     }
     for (uint32_t p = have_pre ? 1 : 0; p < patience; ++p) {
-      if (Ring<F, kUniform, kWarpFaa>::try_enq(r, x, &t, flags) == RING_OK) return;
+      if (cell) {
+        const uint64_t tk = R::take(r.tail);
+        st_relaxed(cell, (tk << 32) | v);
+        if (R::try_enq(r, x | kWfqFast, &t, flags | kRelaxedInstall, true, tk) == RING_OK) return;
+      } else if (R::try_enq(r, x, &t, flags) == RING_OK) return;
       have_t = true;
       ++*retries;
     }
+    if (cell) st_relaxed(cell, (uint64_t)v);                          // slow path: payload before the request is published
     // Seed of the local word: a counter value strictly below every ticket the slow path can
     // obtain (a failed fast ticket, or current - 1), else the local word could return to its
     // seed after round one and a late helper's CAS would re-open that round (ABA).
@@ -371,8 +386,13 @@ __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32
     return FULL;
   }
   ctx.hungry &= ~2u;
-  st_relaxed32(q.data + idx, v);
-  Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags);
+  uint64_t* cell = q.data + idx;
+  if (q.flags & kFencedPayload) {                                   // the paper's scheme: payload, then release-install
+    st_relaxed(cell, (uint64_t)v);
+    Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags);
+  } else {
+    Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags, false, 0, cell, v);
+  }
   return OK;
 }
 
@@ -387,15 +407,24 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
     return EMPTY;
   }
   ctx.hungry &= ~1u;
-  const uint32_t v = ld_relaxed32(q.data + idx);
+  const bool fast = (idx & kWfqFast) != 0;                          // installed by a fast-path enqueue (D6)
+  idx &= kWfqIdxMask;
+  const uint64_t* cell = q.data + idx;
+  uint64_t w = ld_relaxed(cell);
   // D5 as in G-LFQ: the FQ tail ticket is reserved behind the payload load (only when a fast attempt
-  // exists to use it).  D6, FQ side only: the index goes back into FQ after the payload load has
-  // delivered its value (control dependency), so the fast-path install needs no release fence;
-  // the AQ side keeps its fence (no ticket-tag handshake in G-WFQ, D6).
+  // exists to use it).  D6, FQ side: the index goes back into FQ after the payload load has
+  // delivered its value (control dependency), so the fast-path install needs no release fence.
   const bool paired = !(q.flags & kNoPairedFaa) && q.enq_patience != 0 && q.enq_patience != 0xFFFFFFFFu;
   uint64_t t = 0;
   if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq.tail);
-  *out = v;
+  if (fast) {                                                       // tagged cell: wait for the store of THIS tenure of idx
+    const uint32_t tag = (uint32_t)ctx.last_ticket;
+    for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {
+      if (nap) __nanosleep(nap);
+      w = ld_relaxed(cell);
+    }
+  }
+  *out = (uint32_t)w;
   const uint32_t fl = (q.flags & kFencedPayload) ? q.flags : (q.flags | kRelaxedInstall);
   Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, fl, paired, t);
   return OK;

@@ -111,7 +111,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
     L->slot_shift = o->layout == 0 ? 0 : (o->layout == 1 ? 2 : 4);
     L->off_aq = off; off += (size_t)(2 * L->N) * (8u << L->slot_shift);
   } else if (kind == GQ_LFQ || kind == GQ_WFQ) {
-    const uint64_t idx_limit = kind == GQ_LFQ ? 0xFFFFFFFEull : 0x3FFFFFFEull;
+    const uint64_t idx_limit = kind == GQ_LFQ ? 0xFFFFFFFEull : 0x1FFFFFFEull;   // G-WFQ: bit 29 of the Index field marks fast-path installs
     if (capacity >= idx_limit) return GQ_E_INVAL;
     if (kind == GQ_WFQ && k >= WfqFmt::kThrNull) return GQ_E_INVAL;
     L->N = pow2ceil(std::max<uint64_t>(capacity, k));
@@ -120,8 +120,8 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
     const size_t ring_bytes = (size_t)(2 * L->N) * (8u << L->slot_shift);
     L->off_aq = off; off += ring_bytes;
     L->off_fq = off; off += ring_bytes;
-    // G-LFQ: 8 B payload cells (ticket tag + value; D6); G-WFQ: plain uint32 payloads
-    L->off_data = off; off += align_up((size_t)capacity * (kind == GQ_LFQ ? 8 : 4), 256);
+    // 8 B payload cells (ticket tag + value; D6)
+    L->off_data = off; off += align_up((size_t)capacity * 8, 256);
     if (kind == GQ_WFQ) {
       L->off_owner_aq = off; off += (size_t)(2 * L->N) * 8;
       L->off_owner_fq = off; off += (size_t)(2 * L->N) * 8;
@@ -237,6 +237,7 @@ static int format_queue(gq_queue* q, cudaStream_t st) {
   } else if (q->kind == GQ_WFQ) {
     format_ring_kernel<WfqFmt><<<grd, blk, 0, st>>>(q->wfq.aq, slots, 0);
     format_ring_kernel<WfqFmt><<<grd, blk, 0, st>>>(q->wfq.fq, slots, q->capacity);
+    CU(cudaMemsetAsync(q->wfq.data, 0, (size_t)q->capacity * 8, st));
     const unsigned g2 = (q->max_threads + blk - 1) / blk;
     format_wfq_records_kernel<<<g2, blk, 0, st>>>(static_cast<WfqRecord*>(q->wfq.aq.rec), q->max_threads);
     format_wfq_records_kernel<<<g2, blk, 0, st>>>(static_cast<WfqRecord*>(q->wfq.fq.rec), q->max_threads);
@@ -316,7 +317,7 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
   } else if (kind == GQ_WFQ) {
     q->wfq.aq = make_ring(q->base, L, L.off_aq, L.off_owner_aq, 0, L.off_rec);
     q->wfq.fq = make_ring(q->base, L, L.off_fq, L.off_owner_fq, 3, L.off_rec_fq);
-    q->wfq.data = reinterpret_cast<uint32_t*>(q->base + L.off_data);
+    q->wfq.data = reinterpret_cast<uint64_t*>(q->base + L.off_data);
     q->wfq.capacity = (uint32_t)capacity;
     q->wfq.nthreads = k;
     auto pat = [](uint32_t v, uint32_t dflt) { return v == GQ_PATIENCE_ZERO ? 0u : (v ? v : dflt); };
