@@ -354,3 +354,33 @@ def test_soak_past_the_ticket_tag_wrap(kind):
         gq.queue_destroy(q)
     assert r["tot_enq"] + r["tot_deq"] > (1 << 33)
     _conserve(r, left)
+
+
+# ---------------------------------------------------------------- linearizability beyond the tiny config
+@pytest.mark.parametrize("kind,threads,ops,capacity",
+                         [(k, 4096, 8, 8192) for k in BIG + ["G-LFQ-listed"]] +
+                         # k > n.  Not G-LFQ-D: it answers index starvation with thousands of FULL / EMPTY returns,
+                         # and the empty-witness part of the bad-pattern check is not polynomial in those
+                         [(k, 4096, 8, 512) for k in ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-listed"]])
+def test_medium_history_bad_pattern_check(kind, threads, ops, capacity):
+    # 65 536 recorded operations from 4096 threads (128 warps over several SMs), k <= n and k > n (index
+    # starvation: dequeuers of FQ park, D2).  Too large for the exact WGL search at this overlap, but for
+    # histories whose returns are all OK / EMPTY with unique values the bad-pattern characterisation
+    # (oracle.poly) is exact, so OK here IS a linearizability verdict for the unbounded-FIFO part; FULL
+    # returns (possible when k > n) are covered by the capacity lower bound and conservation.
+    q = make(kind, capacity, max_threads=threads, **(dict(ymc_pool_cells=1 << 24) if is_ymc(kind) else {}))
+    try:
+        r = gq.run_balanced(q, threads=threads, ops_per_thread=ops, record_history=1, jitter_ns=100, seed=11)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, capacity + threads + 1)
+    finally:
+        gq.queue_destroy(q)
+    assert len(recs) == threads * ops * 2
+    assert r["tot_empty"] + r["tot_full"] < 256, "parking (D2) should absorb index starvation here"
+    h = to_history(recs)
+    assert oracle.precheck(h) == ""
+    assert oracle.conservation(h, left) == ""
+    pr, why = oracle.poly(h)
+    assert pr == oracle.LIN_OK, why
+    if not is_ymc(kind):
+        assert oracle.capacity_bound(h, capacity + soft_slack(kind, threads)) == ""
