@@ -277,6 +277,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- ceilings at the same occupancy (rank 0, outside the timed region)
     c1 = gq.run_faa_ceiling(1, threads=threads, warmup_ms=5, duration_ms=30)
     c4 = gq.run_faa_ceiling(4, threads=threads, warmup_ms=5, duration_ms=30)
+    c1l = gq.run_faa_ceiling(1, per_lane=True, threads=threads, warmup_ms=5, duration_ms=30)
     c1_tps = c1["succ_enq"] / c1["meas_seconds"]
     c4_tps = c4["succ_enq"] / c4["meas_seconds"]
     peaks, peak_src = measured_peaks()
@@ -294,7 +295,8 @@ def run_ours(args, rank, world, local_rank):
                 "profiles/r1b_balanced_ncu_full.md): the rings are L2-resident, so DRAM sees the cold first touch only; L2 sector bytes per op beside it",
                 "kernel": "gqk::bench_kernel", "kernel_ms": kernel_ms,
                 "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run",
-                "c1_gtickets_s": c1_tps / 1e9, "c4_gtickets_s": c4_tps / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),
+                "c1_gtickets_s": c1_tps / 1e9, "c4_gtickets_s": c4_tps / 1e9,
+                "c1_per_lane_faa_gtickets_s": c1l["succ_enq"] / c1l["meas_seconds"] / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),
                 "algorithmic_GBps": algo_gbps, "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src,
                 "hbm_frac": algo_gbps / peaks["hbm_gbs"]}
 

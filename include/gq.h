@@ -135,6 +135,7 @@ int run_split   (gq_queue* q, const gq_run_cfg* cfg, gq_run_result* res);
 /* Ceiling C1: bare warp-batched FAA (Alg. 1 WAVEFAA) on one counter, nothing else.
    res->succ_enq = tickets taken inside the window.  n_counters in {1,4}: 4 = each warp cycles
    over four padded counters (the like-for-like ceiling for one enqueue+dequeue pair). */
+#define GQ_CEILING_PER_LANE 0x100u   /* OR into n_counters: one FAA per thread (the "naive" loop of P:L95) instead of WAVEFAA */
 int run_faa_ceiling(const gq_run_cfg* cfg, uint32_t n_counters, gq_run_result* res);
 /* Ceiling C2: coalesced stream of 64-bit CAS + red.or over a ring-sized L2-resident buffer. */
 int run_slot_atomic_ceiling(const gq_run_cfg* cfg, uint64_t slots, gq_run_result* res);

@@ -134,7 +134,14 @@ __device__ __forceinline__ void warp_faa2(uint64_t* ca, uint64_t* cb, uint64_t u
   *b = bb + (uint64_t)rank * unit_b;
 }
 // The "naive" per-thread FAA of PAPER.md L95, kept for the ablation (GQ_F_PER_LANE_FAA).
-__device__ __forceinline__ uint64_t lane_faa(uint64_t* counter, uint64_t unit = 1) { return faa_relaxed(counter, unit); }
+// ptxas (12.9, sm_100a) warp-aggregates an atom.add by itself when it can prove the address and the
+// operand warp-uniform (queue views are kernel parameters, so it can): SASS shows an elected lane and
+// one ATOMG.  The term below is always 0 but depends on the thread index, which keeps the address
+// from being provably uniform, so that this really is one FAA per thread.
+__device__ __forceinline__ uint64_t lane_faa(uint64_t* counter, uint64_t unit = 1) {
+  counter += (blockIdx.x * blockDim.x + threadIdx.x) >> 31;
+  return faa_relaxed(counter, unit);
+}
 
 // Same batching for FAA(Threshold, -1) (Alg. 1): lanes of one group get the values
 // a lane-ordered sequence of single decrements would have returned.

@@ -193,9 +193,12 @@ def run_split(q, **kw):
     return res.asdict()
 
 
-def run_faa_ceiling(n_counters=1, **kw):
+GQ_CEILING_PER_LANE = 0x100
+
+
+def run_faa_ceiling(n_counters=1, per_lane=False, **kw):
     res = gq_run_result()
-    _chk(lib.run_faa_ceiling(C.byref(_cfg(**kw)), n_counters, C.byref(res)), "run_faa_ceiling")
+    _chk(lib.run_faa_ceiling(C.byref(_cfg(**kw)), n_counters | (GQ_CEILING_PER_LANE if per_lane else 0), C.byref(res)), "run_faa_ceiling")
     return res.asdict()
 
 

@@ -605,6 +605,8 @@ static int run_ceiling(K kernel, const gq_run_cfg* cfg, gq_run_result* res, uint
 }
 
 extern "C" int run_faa_ceiling(const gq_run_cfg* cfg, uint32_t n_counters, gq_run_result* res) {
+  const bool per_lane = (n_counters & GQ_CEILING_PER_LANE) != 0;
+  n_counters &= ~(uint32_t)GQ_CEILING_PER_LANE;
   if (!cfg || !res || n_counters < 1 || n_counters > 8) return GQ_E_INVAL;
   if (cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
   uint64_t *d_counters = nullptr, *d_ctr = nullptr;
@@ -613,7 +615,8 @@ extern "C" int run_faa_ceiling(const gq_run_cfg* cfg, uint32_t n_counters, gq_ru
   if (e != cudaSuccess) { cudaFree(d_counters); return cuda_fail(e, "cudaMalloc"); }
   cudaMemset(d_counters, 0, 8 * 1024); cudaMemset(d_ctr, 0, C_COUNT * 8);
   void* args[4] = {&d_counters, &n_counters, nullptr, &d_ctr};
-  int rc = run_ceiling(faa_ceiling_kernel<true>, cfg, res, d_ctr, args);
+  int rc = per_lane ? run_ceiling(faa_ceiling_kernel<false>, cfg, res, d_ctr, args)
+                    : run_ceiling(faa_ceiling_kernel<true>, cfg, res, d_ctr, args);
   cudaFree(d_counters); cudaFree(d_ctr);
   return rc;
 }
