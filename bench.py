@@ -285,8 +285,10 @@ def run_ours(args, rank, world, local_rank):
     algo_gbps = ops_per_s_kernel * ALGO_BYTES_PER_OP[args.kind] / 1e9
     traffic, traffic_detail = None, None
     try:
-        traffic_detail = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.kind)
-        traffic = traffic_detail["dram_bytes_per_launch"]      # dram__bytes_read.sum + dram__bytes_write.sum, one launch
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:      # written from the committed ncu captures
+            traffic_detail = next(r for r in csv.DictReader(f) if r["kind"] == args.kind)
+        traffic = float(traffic_detail["dram_bytes_per_launch"])   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
     except Exception:
         pass
     roofline = {"bound": "l2_atomic", "achieved": ops_per_s_kernel / 1e9, "peak": 2 * c1_tps / 1e9, "unit": "Gop/s",
