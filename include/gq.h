@@ -49,7 +49,7 @@ typedef struct {
   uint32_t max_threads;     /* k upper bound: sizes per-thread records and the ring parameter
                                N = max(capacity, pow2ceil(max_threads)) (reading G1);
                                default = full co-residency of the benchmark kernel */
-  uint32_t enq_patience;    /* G-WFQ / YMC fast attempts before the slow path; default 16 / 10 */
+  uint32_t enq_patience;    /* G-WFQ / YMC fast attempts before the slow path; default 64 / 10 */
   uint32_t deq_patience;    /* default 64 / 10 */
   uint32_t help_delay;      /* D: inspect one peer record every D operations; default 64 */
   uint64_t ymc_pool_cells;  /* G-WFQ-YMC preallocated cells; default 2^26 */

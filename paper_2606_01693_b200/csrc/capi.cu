@@ -321,7 +321,7 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
     q->wfq.capacity = (uint32_t)capacity;
     q->wfq.nthreads = k;
     auto pat = [](uint32_t v, uint32_t dflt) { return v == GQ_PATIENCE_ZERO ? 0u : (v ? v : dflt); };
-    q->wfq.enq_patience = pat(q->opts.enq_patience, 16);      // reading W2
+    q->wfq.enq_patience = pat(q->opts.enq_patience, 64);      // reading W2
     q->wfq.deq_patience = pat(q->opts.deq_patience, 64);
     q->wfq.help_delay = q->opts.help_delay ? q->opts.help_delay : 64;   // D = 64
     q->wfq.flags = q->opts.flags;
