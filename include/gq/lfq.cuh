@@ -65,7 +65,7 @@ __device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, u
 // Payload cells (DESIGN.md departure D6, sm_100a).  The paper's scheme (Data[idx] <- v, then publish
 // idx) needs the payload store to be performed before the installing CAS, i.e. a release fence in
 // front of each install: MEMBAR.ALL.GPU, which waits for every outstanding store and reduction of
-// the thread and costs about two extra L2 round trips per operation on B200 (measured: 29 -> 36
+// the thread and costs about two extra L2 round trips per operation on B200 (measured: 31 -> 43
 // Gops/s without them).  Instead each Data cell is one 64-bit word <tag | v>, tag = the low 32 bits
 // of the AQ tail ticket the index is installed under, and the hand-over is a handshake that needs
 // no cross-location ordering:
