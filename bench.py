@@ -299,6 +299,8 @@ def run_ours(args, rank, world, local_rank):
                 "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run",
                 "c1_gtickets_s": c1_tps / 1e9, "c4_gtickets_s": c4_tps / 1e9,
                 "c1_per_lane_faa_gtickets_s": c1l["succ_enq"] / c1l["meas_seconds"] / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),
+                "index_cycle_us": (2.0 * CAPACITY / ops_per_s_kernel * 1e6) if threads > CAPACITY else None,
+                "index_cycle_note": "k > n: the n indices each go FQ -> enqueuer -> AQ -> dequeuer -> FQ; ops/s = 2n / cycle (DESIGN.md section 5)",
                 "algorithmic_GBps": algo_gbps, "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src,
                 "hbm_frac": algo_gbps / peaks["hbm_gbs"]}
 
