@@ -166,7 +166,7 @@ int history_dump(gq_queue* q, gq_hist_rec* host_out, uint64_t max, uint64_t* n_o
 typedef struct {
   uint32_t threads;        /* participating threads (P:L365 sweeps 2^9..2^13); 0 = full co-residency */
   uint32_t block_threads;  /* 0 = 256 */
-  uint32_t huge_degree;    /* adjacency lists at least this long are expanded by the whole grid; 0 = 1024 */
+  uint32_t huge_degree;    /* adjacency lists at least this long are expanded by the whole grid; 0 = 64 (also the minimum) */
   uint32_t flags;          /* GQ_F_* for the two queues */
 } gq_bfs_opts;
 typedef struct { uint32_t levels; uint32_t threads; uint64_t edges_scanned, vertices_visited, queue_ops; double ms, total_ms; } gq_bfs_stats;
