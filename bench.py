@@ -334,6 +334,16 @@ def run_ours(args, rank, world, local_rank):
                                     "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1),
                                     "full_rate": round(r["full"] / max(1, r["full"] + r["succ_enq"]), 4),
                                     "empty_rate": round(r["empty"] / max(1, r["empty"] + r["succ_deq"]), 4)}
+                if name == "lfq":       # the same roles with homogeneous warps (gq_run_cfg.role_layout = 1): how much of
+                    ptc = {}            # the split deficit is SIMT divergence inside mixed warps, not the queue
+                    for pf in (0.25, 0.5, 0.75):
+                        gq.queue_reset(qq)
+                        gq.queue_prefill(qq, pre)
+                        r = gq.run_split(qq, threads=fk, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=pf,
+                                         seed=1, value_base=1 << 19, role_layout=1)
+                        ptc[str(pf)] = {"enq_mops": round(r["succ_enq"] / r["meas_seconds"] / 1e6, 1),
+                                        "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1)}
+                    sweep["split_lfq_role_layout_1"] = ptc
                 gq.queue_destroy(qq)
                 sweep["split_" + name] = pts
             except gq.GqError as e:

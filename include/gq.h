@@ -115,6 +115,10 @@ typedef struct {
   uint32_t jitter_ns;          /* random __nanosleep in [0, jitter_ns] before each op (history runs) */
   uint32_t fail_backoff_ns;    /* harness sleeps up to this long after a FULL/EMPTY return (0 = none) */
   uint64_t value_base;         /* first payload value (split: prefill size) */
+  uint32_t role_layout;        /* run_split: 0 = logical thread t runs on physical thread t (mixed warps, the default);
+                                  1 = same seeded roles, but the logical threads are placed so that producers fill the
+                                  first physical threads and consumers the rest: warps are homogeneous (at most one mixed) */
+  uint32_t reserved;           /* must be 0 */
 } gq_run_cfg;
 
 typedef struct {

@@ -41,7 +41,8 @@ class gq_run_cfg(C.Structure):
     _fields_ = [("threads", C.c_uint32), ("block_threads", C.c_uint32), ("warmup_ms", C.c_double),
                 ("duration_ms", C.c_double), ("producer_fraction", C.c_double), ("seed", C.c_uint64),
                 ("record_history", C.c_uint32), ("ops_per_thread", C.c_uint32), ("jitter_ns", C.c_uint32),
-                ("fail_backoff_ns", C.c_uint32), ("value_base", C.c_uint64)]
+                ("fail_backoff_ns", C.c_uint32), ("value_base", C.c_uint64),
+                ("role_layout", C.c_uint32), ("reserved", C.c_uint32)]
 
 
 class gq_run_result(C.Structure):

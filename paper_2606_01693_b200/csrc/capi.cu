@@ -31,7 +31,7 @@ static int cuda_fail(cudaError_t e, const char* what) { return gq_cuda_fail(e, w
 extern "C" const char* gq_last_cuda_error(void) { return g_err; }
 extern "C" const char* gq_version(void) { return "gq 0.1 (sm_100a)"; }
 
-static_assert(sizeof(gq_opts) == 56 && sizeof(gq_run_cfg) == 64 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
+static_assert(sizeof(gq_opts) == 56 && sizeof(gq_run_cfg) == 72 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
               "ABI structs: the Python binding mirrors these layouts");
 
 // ------------------------------------------------------------------------------- handle
@@ -555,17 +555,32 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   BenchParams p = make_params(cfg, r, mode);
   Q v = view;
   set_nthreads(v, r.threads);          // help ring = the launched threads (reading W7)
+  uint32_t* d_perm = nullptr;
+  if (mode == MODE_SPLIT && cfg->role_layout == 1) {   // same seeded roles, producers first: homogeneous warps
+    std::vector<uint32_t> perm; perm.reserve(r.threads);
+    std::vector<uint32_t> cons; cons.reserve(r.threads);
+    for (uint32_t t = 0; t < r.threads; ++t)
+      ((uint64_t)gq::detail::mix32(p.seed * 0x9e3779b9u + t) < p.prod_threshold ? perm : cons).push_back(t);
+    perm.insert(perm.end(), cons.begin(), cons.end());
+    CU(cudaMalloc(&d_perm, (size_t)r.threads * 4));
+    cudaError_t ce = cudaMemcpy(d_perm, perm.data(), (size_t)r.threads * 4, cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) { cudaFree(d_perm); return cuda_fail(ce, "memcpy(perm)"); }
+    p.perm = d_perm;
+  } else if (cfg->role_layout > 1) {
+    return GQ_E_INVAL;
+  }
   uint64_t* ctr = q->d_ctr; gq_hist_rec* h = q->d_hist;
   void* args[] = {&v, &p, &ctr, &h};
   cudaEvent_t e0, e1;
   CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
   CU(cudaEventRecord(e0, nullptr));
   cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
-  if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return le == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : cuda_fail(le, "launch"); }
+  if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); if (d_perm) cudaFree(d_perm); return le == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : cuda_fail(le, "launch"); }
   CU(cudaEventRecord(e1, nullptr));
   rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
   if (rc == 0) rc = finish_run(q->d_ctr, e0, e1, cfg, r, res);
   cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (d_perm) cudaFree(d_perm);
   if (rc == 0) report_stuck();
   if (rc == 0) rc = collect_stats(q, res);
   if (rc == 0 && res->pool_exhausted) return GQ_E_POOL;

@@ -25,6 +25,7 @@ struct BenchParams {
   uint32_t seed, ops_per_thread;
   uint32_t jitter_ns, fail_backoff_ns;
   uint64_t value_base;
+  const uint32_t* perm;        // physical -> logical thread id (role_layout 1), or nullptr
 };
 
 __device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
@@ -49,29 +50,30 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
   uint64_t sum_enq = 0, sum_deq = 0, retries = 0;
 
   if (tid < p.threads) {
-    thread_ctx ctx{tid};
-    ctx.help_peer = tid + 1;
+    const uint32_t ltid = p.perm ? p.perm[tid] : tid;      // logical thread (roles, payloads, records); tid = physical
+    thread_ctx ctx{ltid};
+    ctx.help_peer = ltid + 1;
     bool do_enq = true, do_deq = true;
     if (p.mode == MODE_SPLIT) {
-      do_enq = (uint64_t)mix32(p.seed * 0x9e3779b9u + tid) < p.prod_threshold;
+      do_enq = (uint64_t)mix32(p.seed * 0x9e3779b9u + ltid) < p.prod_threshold;
       do_deq = !do_enq;
     }
     const uint32_t per_iter = p.mode == MODE_SPLIT ? 1 : 2;
-    gq_hist_rec* my = kHist ? hist + (size_t)tid * p.ops_per_thread * per_iter : nullptr;
+    gq_hist_rec* my = kHist ? hist + (size_t)ltid * p.ops_per_thread * per_iter : nullptr;
     uint32_t fail_ns = 0;
     for (uint32_t iter = 0;; ++iter) {
       uint64_t now = 0;
       if (do_enq) {
-        const uint32_t v = (uint32_t)(p.value_base + tid + (uint64_t)iter * p.threads);
+        const uint32_t v = (uint32_t)(p.value_base + ltid + (uint64_t)iter * p.threads);
         uint64_t t_call = 0;
         if (kHist) {
-          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (tid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
+          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
           t_call = globaltimer_ns();
         }
         const int s = enqueue<true, kWarpFaa>(q, ctx, v, &retries);
         if (kHist) { __threadfence(); }               // effects performed before `end` is read (reading H1)
         now = globaltimer_ns();
-        if (kHist) *my++ = gq_hist_rec{tid, GQ_OP_ENQ, v, (uint32_t)s, 0u, 0u, t_call, now};
+        if (kHist) *my++ = gq_hist_rec{ltid, GQ_OP_ENQ, v, (uint32_t)s, 0u, 0u, t_call, now};
         const bool in = now >= tw && now < te;
         if (s == OK) { ++tot_enq; sum_enq += v; succ_enq += in; fail_ns = 0; }
         else {
@@ -83,13 +85,13 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
         uint32_t v = 0;
         uint64_t t_call = 0;
         if (kHist) {
-          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (tid * 0xc2b2ae35u) ^ (iter * 2u + 0x7654321u)) % (p.jitter_ns + 1));
+          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0xc2b2ae35u) ^ (iter * 2u + 0x7654321u)) % (p.jitter_ns + 1));
           t_call = globaltimer_ns();
         }
         const int s = dequeue<true, kWarpFaa>(q, ctx, &v, &retries);
         if (kHist) { __threadfence(); }
         now = globaltimer_ns();
-        if (kHist) *my++ = gq_hist_rec{tid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
+        if (kHist) *my++ = gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
         const bool in = now >= tw && now < te;
         if (s == OK) { ++tot_deq; sum_deq += v; succ_deq += in; fail_ns = 0; }
         else {

@@ -384,3 +384,37 @@ def test_medium_history_bad_pattern_check(kind, threads, ops, capacity):
     assert pr == oracle.LIN_OK, why
     if not is_ymc(kind):
         assert oracle.capacity_bound(h, capacity + soft_slack(kind, threads)) == ""
+
+
+# ---------------------------------------------------------------- split with compacted roles
+@pytest.mark.parametrize("kind", ["G-LFQ", "G-WFQ", "G-WFQ-YMC"])
+def test_split_role_layout_compact(kind):
+    # role_layout = 1 (gq.h): the same seeded Bernoulli roles, but logical threads are placed so that warps are
+    # homogeneous.  Same logical behaviour: tiny history through the checker, then BJ config 3 shape conserving.
+    q = make(kind, 16, max_threads=64, park_ns=1000)
+    try:
+        r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1, jitter_ns=200, seed=3,
+                         producer_fraction=0.5, role_layout=1)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, 2048)
+    finally:
+        gq.queue_destroy(q)
+    assert len(recs) == 1024 and sorted(set(recs["proc"].tolist())) == list(range(64))
+    # a logical thread is a pure producer or a pure consumer, as drawn from the seed
+    for t in range(64):
+        assert len(set(recs["op"][recs["proc"] == t].tolist())) == 1
+    ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 16), relaxed_full=True, leftover=left,
+                                   max_steps=3_000_000, accept_unknown=True)
+    assert ok, msg
+    n = 1 << 20
+    pre = np.arange(n // 2, dtype=np.uint32)
+    ymc = is_ymc(kind)
+    q = make(kind, n, **(dict(ymc_pool_cells=1 << 28) if ymc else {}))
+    try:
+        gq.queue_prefill(q, pre)
+        kw = dict(ops_per_thread=40) if ymc else dict(warmup_ms=2, duration_ms=10)
+        r = gq.run_split(q, threads=0, producer_fraction=0.5, seed=7, value_base=n // 2, role_layout=1, **kw)
+        left = gq.queue_drain(q, (1 << 24) if ymc else n + 1)
+    finally:
+        gq.queue_destroy(q)
+    _conserve(r, left, pre)
