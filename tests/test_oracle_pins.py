@@ -274,3 +274,32 @@ def test_soft_capacity_mode_for_the_direct_payload_ablation():
     # FIFO order is untouched by the soft bound
     rows = [(0, E, 7, 0, 0, 0, 1), (1, E, 8, 0, 0, 2, 3), (0, D, 0, 0, 8, 20, 21)]
     assert oracle.brute(H(rows), 4, 2) == LIN_VIOLATION
+
+
+# ------------------------------------------------------------------ tests/golden: hand-derived verdicts
+def _golden():
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "histories.txt")
+    out = []
+    for ln in open(path):
+        ln = ln.strip()
+        if not ln or ln.startswith("#"):
+            continue
+        verdict, cap, relaxed, ops, note = [x.strip() for x in ln.split("|")]
+        rows = []
+        for o in ops.split(";"):
+            proc, op, arg, status, val, call, end = o.split()
+            rows.append((int(proc), E if op == "E" else D, int(arg), {"OK": ST_OK, "FULL": ST_FULL, "EMPTY": ST_EMPTY}[status],
+                         int(val), int(call), int(end)))
+        out.append((note, rows, int(cap), int(relaxed), LIN_OK if verdict == "LIN" else LIN_VIOLATION))
+    return out
+
+
+@pytest.mark.parametrize("note,rows,cap,relaxed,expected", _golden(), ids=[g[0][:40] for g in _golden()])
+def test_golden_histories(note, rows, cap, relaxed, expected):
+    h = H(rows)
+    assert oracle.brute(h, cap, relaxed) == expected, note
+    assert oracle.wgl(h, cap, relaxed)[0] == expected, note
+    pr, why = oracle.poly(h)
+    if pr == LIN_VIOLATION:                      # the polynomial refuter must never reject a linearizable history
+        assert expected == LIN_VIOLATION, (note, why)
