@@ -181,6 +181,16 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
   for (uint32_t p = 0; p < q.enq_patience; ++p) {
     const uint64_t i = Y::take<kUniform, kWarpFaa>(q.tail);
     if (i >= Y::last(q)) { Y::pool_exhausted(q); return FULL; }
+    // Cells are never reused, so every deposit CAS would be the first touch of its line: an L2 miss
+    // that the atomic unit of that slice waits out, and with it every other atomic queued there, the FAAs on
+    // H and T included (ncu: the wait for the dequeue's FAA was 9x that of the enqueue's).  Tickets are
+    // sequential, so the line a later wave of tickets will use is known: pull it into L2 one wave
+    // (k tickets) ahead.  A hint only; GQ_F_NO_CELL_PREFETCH switches it off.  Measured on B200:
+    // 28.4 -> 43.9 Gops/s at 65 536 threads, 24.8 -> 39.6 at full co-residency.
+    if (!(q.flags & kNoCellPrefetch)) {
+      const uint64_t j = i + q.nthreads;
+      if (j < Y::last(q)) asm volatile("prefetch.global.L2 [%0];" :: "l"(q.pool + j));
+    }
     // relaxed: the word carries the payload itself and the fast path has published nothing else
     // (the slow path's request record keeps its release/acquire discipline)
     if (cas_relaxed(&Y::cell(q, i)->val, Y::kBot, val) == Y::kBot) return OK;
