@@ -29,7 +29,7 @@ struct RingView {
   uint32_t  park_ns;    // D2: longest time a dequeuer waits on its own vacant slot (0 = never)
   uint32_t  park_limit; // D1: EMPTY without a ticket once Head is this far ahead of Tail
   uint32_t  park_nap;   // D2: longest single __nanosleep between two looks at the parked slot
-  uint32_t  _pad;
+  uint32_t  prefetch;   // > 0: rings too large to stay L2-resident: pull the slot `prefetch` tickets ahead into L2
 };
 
 namespace detail {
@@ -207,6 +207,9 @@ struct Ring {
                                                 bool have = false, uint64_t t_pre = 0) {
     const uint64_t t = have ? t_pre : take(r.tail);                   // L144
     *t_out = t;
+    // A first-touch CAS is an L2 miss that the slice's atomic unit waits out, with every atomic queued behind
+    // it ("cold lines"): for rings that cannot stay L2-resident, fetch a later slot now.
+    if (r.prefetch) asm volatile("prefetch.global.L2 [%0];" :: "l"(slot(r, slot_of(r, t + r.prefetch))));
     const uint32_t j = slot_of(r, t), c = cycle_of(r, t);             // L146
     uint64_t* sp = slot(r, j);
     uint64_t E;
@@ -284,6 +287,7 @@ struct Ring {
       h = take(r.head);                                               // L172
     }
     *h_out = h;
+    if (r.prefetch) asm volatile("prefetch.global.L2 [%0];" :: "l"(slot(r, slot_of(r, h + r.prefetch))));
     const uint32_t j = slot_of(r, h), c = cycle_of(r, h);             // L175
     uint64_t* sp = slot(r, j);
     uint32_t waited = 0, nap = r.park_nap < 32 ? r.park_nap : 32;

@@ -86,7 +86,7 @@ struct Layout {
   size_t off_hot = 0, off_aq = 0, off_fq = 0, off_data = 0, off_owner_aq = 0, off_owner_fq = 0, off_rec = 0, off_rec_fq = 0, off_pool = 0;
   size_t total = 0;
   uint64_t pool_cells = 0;
-  uint32_t park_ns = 0, park_nap = 0;
+  uint32_t park_ns = 0, park_nap = 0, prefetch_dist = 0;
 };
 
 template <class Q> static int max_blocks_per_sm(int block_threads);
@@ -102,6 +102,7 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   *max_threads_out = k;
   L->park_ns = o->park_ns ? o->park_ns : 250000u;
   L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 128u;
+  L->prefetch_dist = (o->flags & GQ_F_NO_CELL_PREFETCH) ? 0u : k;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
   if (kind == GQ_LFQ_DIRECT) {                        // one ring, payload in the entry word: no FQ, no Data
@@ -178,6 +179,9 @@ static RingView make_ring(char* base, const Layout& L, size_t off_entries, size_
   r.park_ns = L.park_ns;
   r.park_nap = L.park_nap;
   r.park_limit = (uint32_t)std::min<uint64_t>(L.N / 2, 0x7FFFFFFFu);
+  // rings of 32 MiB and more (BFS frontier queues) do not stay in L2 next to the graph: prefetch k tickets ahead
+  const size_t ring_bytes = (size_t)(2 * L.N) * (8u << L.slot_shift);
+  r.prefetch = ring_bytes >= (32u << 20) ? L.prefetch_dist : 0;
   return r;
 }
 
