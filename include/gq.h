@@ -78,6 +78,9 @@ enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the w
                                    and parks (D2) only for an enqueuer that already holds its ticket; the default waits
                                    in line for future enqueues, which is what the fixed-duration benchmarks want */
        GQ_F_NO_CELL_PREFETCH = 1024u, /* ablation: G-WFQ-YMC enqueue does not prefetch the pool cells of the next ticket wave into L2 */
+       GQ_F_NO_FULL_TEST = 2048u, /* G-LFQ-D only: the caller guarantees that the queue never holds `capacity` items (a BFS
+                                   frontier queue of nv slots, a work queue of all items): enqueue skips the FULL test, which is
+                                   the two hot-word loads that make G-LFQ-D slow at scale */
        GQ_F_FENCED_PAYLOAD = 256u /* G-LFQ: order the payload against the index hand-over with release fences in front of
                                    both installing CAS (the paper's implicit scheme) instead of the payload-cell
                                    handshake (D6) */ };

@@ -37,7 +37,7 @@ namespace detail {
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
 enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
-                  kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u, kEagerEmpty = 512u, kNoCellPrefetch = 1024u,
+                  kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u, kEagerEmpty = 512u, kNoCellPrefetch = 1024u, kNoFullTest = 2048u,
                   kRelaxedInstall = 1u << 16 /* internal: this install needs no release edge */ };
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index

@@ -25,9 +25,11 @@ template <bool kUniform = false, bool kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const DlfqView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
-  const uint64_t H = ld_relaxed(q.r.head);                          // Head first: a later Tail can only overstate the fill,
-  const uint64_t T = ld_relaxed(q.r.tail);                          // by dequeues that overlap this operation
-  if (T >= H + q.capacity) { ctx.hungry |= 2u; return FULL; }
+  if (!(q.flags & kNoFullTest)) {                                   // GQ_F_NO_FULL_TEST: the caller bounds the fill itself
+    const uint64_t H = ld_relaxed(q.r.head);                        // Head first: a later Tail can only overstate the fill,
+    const uint64_t T = ld_relaxed(q.r.tail);                        // by dequeues that overlap this operation
+    if (T >= H + q.capacity) { ctx.hungry |= 2u; return FULL; }
+  }
   ctx.hungry &= ~2u;
   // relaxed install: the entry word is the payload, there is nothing else to publish
   ring_enq_loop<DirFmt, kUniform, kWarpFaa>(q.r, v, retries, q.flags | kRelaxedInstall);

@@ -18,7 +18,7 @@ GQ_OP_ENQ, GQ_OP_DEQ = 0, 1
 GQ_E_INVAL, GQ_E_NOMEM, GQ_E_CUDA, GQ_E_RESIDENCY, GQ_E_TIMEOUT, GQ_E_STATE, GQ_E_POOL = -1, -2, -3, -4, -5, -6, -7
 GQ_PATIENCE_ZERO = 0xFFFFFFFF
 GQ_F_PER_LANE_FAA, GQ_F_NO_PROBE, GQ_F_NO_DEQ_SPIN, GQ_F_NO_OPT_CAS, GQ_F_PLAIN_THR_STORE = 1, 2, 4, 8, 16
-GQ_F_THR_FIRST, GQ_F_NO_PAIRED_FAA, GQ_F_THR_RED_MAX, GQ_F_FENCED_PAYLOAD, GQ_F_EAGER_EMPTY, GQ_F_NO_CELL_PREFETCH = 32, 64, 128, 256, 512, 1024
+GQ_F_THR_FIRST, GQ_F_NO_PAIRED_FAA, GQ_F_THR_RED_MAX, GQ_F_FENCED_PAYLOAD, GQ_F_EAGER_EMPTY, GQ_F_NO_CELL_PREFETCH, GQ_F_NO_FULL_TEST = 32, 64, 128, 256, 512, 1024, 2048
 KIND_NAMES = {GQ_LFQ: "G-LFQ", GQ_WFQ: "G-WFQ", GQ_WFQ_YMC: "G-WFQ-YMC", GQ_LFQ_DIRECT: "G-LFQ-D"}
 _ERR = {-1: "INVAL", -2: "NOMEM", -3: "CUDA", -4: "RESIDENCY", -5: "TIMEOUT", -6: "STATE", -7: "POOL"}
 
