@@ -319,6 +319,8 @@ def run_ours(args, rank, world, local_rank):
                 gq.queue_reset(qq)
                 r = gq.run_balanced(qq, threads=th, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns)
                 pts[str(th)] = round(r["mops"], 1)
+                if r["pool_exhausted"]:
+                    pts[str(th) + "_pool_exhausted"] = True      # G-WFQ-YMC ran out of cells inside the run: the number is low
             gq.queue_destroy(qq)
             sweep["balanced_" + name] = pts
             try:
