@@ -387,6 +387,9 @@ def run_ours(args, rank, world, local_rank):
         "gpu_launches": args.steps * 3,      # per step: 2 format kernels (queue_reset) + 1 bench kernel
         "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline, "sweep": sweep,
         "conservation": "checked every e2e step: tot_enq - tot_deq == drained",
+        # P:L359 protocol ("5 runs, median"): the timed steps one by one (rank 0's replica) and their median
+        "per_step_mops": [round((r["succ_enq"] + r["succ_deq"]) / (DURATION_MS * 1e-3) / 1e6, 1) for r in results],
+        "median_step_mops": round(statistics.median((r["succ_enq"] + r["succ_deq"]) / (DURATION_MS * 1e-3) / 1e6 for r in results), 1),
     }
     if apps is not None:
         line["apps"] = apps
