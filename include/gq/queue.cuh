@@ -4,7 +4,7 @@
 //   int s = gq::enqueue(view, ctx, v);             // gq::OK | gq::FULL
 //   int s = gq::dequeue(view, ctx, &v);            // gq::OK | gq::EMPTY
 //
-// `view` is the POD LfqView / WfqView / YmcView obtained on the host with
+// `view` is the POD LfqView / WfqView / YmcView (or DlfqView, the direct-payload ablation) obtained on the host with
 // queue_device_view() (gq.h) and passed to the kernel by value.  Any subset of lanes may
 // call, converged or diverged.  Template flag kUniform = true promises that all lanes
 // converged at the call use the same queue (skips the address match in warp_faa).
