@@ -336,8 +336,8 @@ def run_ours(args, rank, world, local_rank):
                                     "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1),
                                     "full_rate": round(r["full"] / max(1, r["full"] + r["succ_enq"]), 4),
                                     "empty_rate": round(r["empty"] / max(1, r["empty"] + r["succ_deq"]), 4)}
-                if name == "lfq":       # the same roles with homogeneous warps (gq_run_cfg.role_layout = 1): how much of
-                    ptc = {}            # the split deficit is SIMT divergence inside mixed warps, not the queue
+                if name == "lfq":       # the same seeded roles placed on homogeneous warps (gq_run_cfg.role_layout = 1):
+                    ptc = {}            # full-size WAVEFAA batches; context for the mixed-warp numbers above
                     for pf in (0.25, 0.5, 0.75):
                         gq.queue_reset(qq)
                         gq.queue_prefill(qq, pre)

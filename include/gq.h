@@ -121,7 +121,9 @@ typedef struct {
   uint64_t value_base;         /* first payload value (split: prefill size) */
   uint32_t role_layout;        /* run_split: 0 = logical thread t runs on physical thread t (mixed warps, the default);
                                   1 = same seeded roles, but the logical threads are placed so that producers fill the
-                                  first physical threads and consumers the rest: warps are homogeneous (at most one mixed) */
+                                  first physical threads and consumers the rest: warps are homogeneous (at most one mixed);
+                                  2 = layout 0, but each iteration is ONE converged call of the fused operation
+                                  gq::enqueue_or_dequeue (G-LFQ only): the two roles of a mixed warp overlap */
   uint32_t reserved;           /* must be 0 */
 } gq_run_cfg;
 

@@ -148,4 +148,54 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
   return OK;
 }
 
+
+// Fused operation for warps whose lanes have different roles (BASELINE.json config 3: the role of every
+// thread is drawn from the seed, so every warp is a mix of producers and consumers).  Called as two
+// separate operations the two groups of a warp run one after the other (SIMT divergence) and their
+// WAVEFAA batches are half-size.  But on the rings the two operations are the same program:
+//     enqueue: ring_deq(FQ) -> payload store -> ring_enq(AQ)      dequeue: ring_deq(AQ) -> payload load -> ring_enq(FQ)
+// so here every lane selects its (first ring, second ring) pair and the whole warp stays converged;
+// the address-matched WAVEFAA (warp_faa<false>, reading G10) elects one leader per counter inside the
+// converged warp, both leaders issue their FAA in the same instruction, and the L2 round trips of the
+// two roles overlap.  *v is the payload (in) for is_enq lanes and the result (out) for the others.
+// Returns OK, FULL (enqueue lanes) or EMPTY (dequeue lanes).  Ticket-tagged cells (D6) only; with
+// GQ_F_FENCED_PAYLOAD it falls back to the two separate calls.
+template <bool kWarpFaa = true>
+__device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& ctx, bool is_enq, uint32_t* v, uint64_t* retries = nullptr) {
+  using namespace detail;
+  using R = Ring<LfqFmt, false, kWarpFaa>;
+  uint64_t dummy = 0; if (!retries) retries = &dummy;
+  if (q.flags & kFencedPayload) return is_enq ? enqueue<false, kWarpFaa>(q, ctx, *v, retries) : dequeue<false, kWarpFaa>(q, ctx, v, retries);
+  RingView r1 = is_enq ? q.fq : q.aq, r2 = is_enq ? q.aq : q.fq;        // per-lane ring pair
+  const uint32_t hbit = is_enq ? 2u : 1u;
+  uint32_t idx;
+  uint64_t h1 = 0;
+  if (ring_deq_loop<LfqFmt, false, kWarpFaa>(r1, &idx, retries, NoFinalize{}, (ctx.hungry & hbit) != 0, q.flags, &h1) == RING_EMPTY) {
+    ctx.hungry |= hbit;
+    return is_enq ? FULL : EMPTY;
+  }
+  ctx.hungry &= ~hbit;
+  if (!is_enq) ctx.last_ticket = h1;
+  uint64_t* cell = q.data + idx;
+  uint64_t w = is_enq ? 0 : ld_relaxed(cell);
+  Backoff bo;
+  for (bool first = true;; first = false) {
+    const uint64_t t = R::take(r2.tail);                               // two leaders, one instruction
+    if (is_enq) {
+      st_relaxed(cell, (t << 32) | *v);                                // D6: payload tagged with its AQ ticket
+    } else if (first) {
+      const uint32_t tag = (uint32_t)h1;
+      for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {
+        if (nap) __nanosleep(nap);
+        w = ld_relaxed(cell);
+      }
+      *v = (uint32_t)w;
+    }
+    uint64_t tt;
+    if (R::try_enq(r2, idx, &tt, q.flags | kRelaxedInstall, true, t) == RING_OK) return OK;
+    ++*retries;
+    bo.pause();
+  }
+}
+
 }  // namespace gq

@@ -536,7 +536,10 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   const bool hist = cfg->record_history != 0;
   if (hist && cfg->ops_per_thread == 0) return GQ_E_INVAL;
   if (!hist && cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
-  void* fn = hist ? (per_lane ? (void*)bench_kernel<Q, true, false> : (void*)bench_kernel<Q, true, true>)
+  const bool fused = mode == MODE_SPLIT && cfg->role_layout == 2;       // mixed warps, one converged call (G-LFQ)
+  if (fused && (q->kind != GQ_LFQ || per_lane)) return GQ_E_INVAL;
+  void* fn = fused ? (hist ? (void*)bench_kernel<Q, true, true, true> : (void*)bench_kernel<Q, false, true, true>)
+           : hist ? (per_lane ? (void*)bench_kernel<Q, true, false> : (void*)bench_kernel<Q, true, true>)
                   : (per_lane ? (void*)bench_kernel<Q, false, false> : (void*)bench_kernel<Q, false, true>);
   Resolved r;
   int nb = 0;
@@ -570,7 +573,9 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
     cudaError_t ce = cudaMemcpy(d_perm, perm.data(), (size_t)r.threads * 4, cudaMemcpyHostToDevice);
     if (ce != cudaSuccess) { cudaFree(d_perm); return cuda_fail(ce, "memcpy(perm)"); }
     p.perm = d_perm;
-  } else if (cfg->role_layout > 1) {
+  } else if (mode == MODE_SPLIT && cfg->role_layout == 2) {
+    p.fused = 1;
+  } else if (cfg->role_layout != 0 && mode == MODE_SPLIT) {
     return GQ_E_INVAL;
   }
   uint64_t* ctr = q->d_ctr; gq_hist_rec* h = q->d_hist;

@@ -26,7 +26,18 @@ struct BenchParams {
   uint32_t jitter_ns, fail_backoff_ns;
   uint64_t value_base;
   const uint32_t* perm;        // physical -> logical thread id (role_layout 1), or nullptr
+  uint32_t fused, _pad;        // role_layout 2: mixed warps call the fused enqueue_or_dequeue (G-LFQ)
 };
+
+// the fused mixed-warp operation exists for G-LFQ (lfq.cuh); other kinds run the two calls
+template <class Q> struct HasFused { static constexpr bool value = false; };
+template <> struct HasFused<LfqView> { static constexpr bool value = true; };
+template <bool kWarpFaa, class Q>
+__device__ __forceinline__ int fused_op(const Q&, thread_ctx&, bool, uint32_t*, uint64_t*) { return -1; }
+template <bool kWarpFaa>
+__device__ __forceinline__ int fused_op(const LfqView& q, thread_ctx& ctx, bool is_enq, uint32_t* v, uint64_t* retries) {
+  return enqueue_or_dequeue<kWarpFaa>(q, ctx, is_enq, v, retries);
+}
 
 __device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
 #pragma unroll
@@ -35,7 +46,7 @@ __device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
 }
 
 // One kernel for both micro-benchmarks.  kHist: record {proc,op,arg,ret,call,end} per op.
-template <class Q, bool kHist, bool kWarpFaa>
+template <class Q, bool kHist, bool kWarpFaa, bool kFused = false>
 __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint64_t* ctr, gq_hist_rec* hist) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -63,6 +74,25 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
     uint32_t fail_ns = 0;
     for (uint32_t iter = 0;; ++iter) {
       uint64_t now = 0;
+      if (kFused && HasFused<Q>::value) {                   // split mode, mixed warps, one converged call per iteration
+        uint32_t v = (uint32_t)(p.value_base + ltid + (uint64_t)iter * p.threads);
+        const uint32_t v_in = v;
+        uint64_t t_call = 0;
+        if (kHist) {
+          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
+          t_call = globaltimer_ns();
+        }
+        const int s = fused_op<kWarpFaa>(q, ctx, do_enq, &v, &retries);
+        if (kHist) { __threadfence(); }
+        now = globaltimer_ns();
+        if (kHist) *my++ = do_enq ? gq_hist_rec{ltid, GQ_OP_ENQ, v_in, (uint32_t)s, 0u, 0u, t_call, now}
+                                  : gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
+        const bool in = now >= tw && now < te;
+        if (do_enq) { if (s == OK) { ++tot_enq; sum_enq += v_in; succ_enq += in; } else { ++tot_full; full += in; } }
+        else        { if (s == OK) { ++tot_deq; sum_deq += v; succ_deq += in; } else { ++tot_empty; empty += in; } }
+        if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
+        continue;
+      }
       if (do_enq) {
         const uint32_t v = (uint32_t)(p.value_base + ltid + (uint64_t)iter * p.threads);
         uint64_t t_call = 0;

@@ -409,6 +409,28 @@ def test_split_role_layout_compact(kind):
     ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 16), relaxed_full=True, leftover=left,
                                    max_steps=3_000_000, accept_unknown=True)
     assert ok, msg
+    if kind == "G-LFQ":
+        # role_layout = 2: mixed warps through the fused gq::enqueue_or_dequeue (address-matched WAVEFAA inside a
+        # converged warp, reading G10); FULL- and EMPTY-heavy tiny histories through the checker
+        for pf, seed in ((0.25, 1), (0.75, 2), (0.5, 3)):
+            q = make(kind, 16, max_threads=64, park_ns=1000)
+            try:
+                r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1, jitter_ns=200,
+                                 seed=seed, producer_fraction=pf, role_layout=2)
+                recs = gq.history_dump(q)
+                left = gq.queue_drain(q, 2048)
+            finally:
+                gq.queue_destroy(q)
+            ok, msg = oracle.check_history(to_history(recs), 16, relaxed_full=True, leftover=left, max_steps=3_000_000,
+                                           accept_unknown=True)
+            assert ok, msg
+    else:
+        q = make(kind, 16, max_threads=64)
+        try:
+            with pytest.raises(gq.GqError):                       # the fused operation exists for G-LFQ only
+                gq.run_split(q, threads=64, block_threads=64, ops_per_thread=4, producer_fraction=0.5, role_layout=2)
+        finally:
+            gq.queue_destroy(q)
     n = 1 << 20
     pre = np.arange(n // 2, dtype=np.uint32)
     ymc = is_ymc(kind)
