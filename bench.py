@@ -351,6 +351,16 @@ def run_ours(args, rank, world, local_rank):
             except gq.GqError as e:
                 sweep["split_" + name] = str(e)
 
+    if not args.no_sweep:
+        # capacity sweep at full co-residency (G-LFQ): for n < k the throughput is 2n / (index cycle), DESIGN.md section 5
+        pts = {}
+        for logn in (13, 14, 15, 16, 17, 18, 20):
+            qq = gq.queue_create(0, 1 << logn)
+            r = gq.run_balanced(qq, threads=full, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS)
+            gq.queue_destroy(qq)
+            pts[f"2^{logn}"] = {"mops": round(r["mops"], 1), "index_cycle_us": round(2.0 * (1 << logn) / (r["mops"] * 1e6) * 1e6, 2) if (1 << logn) < full else None}
+        sweep["capacity_lfq_full_coresidency"] = pts
+
     apps = None
     if args.apps:
         apps = run_apps(gq, torch, args.apps_scale)
