@@ -34,6 +34,13 @@ struct RingView {
 
 namespace detail {
 
+#ifdef GQ_DBG_SITES
+static __device__ unsigned long long g_dbg[32];
+#define GQ_SITE(i) atomicAdd(&g_dbg[i], 1ull)
+#else
+#define GQ_SITE(i) ((void)0)
+#endif
+
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
 enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
@@ -233,6 +240,10 @@ struct Ring {
         reset_threshold(r, flags);                                    // L155
         return RING_OK;
       }
+      GQ_SITE(ok ? 0 : 1);                                            // 0: second CAS lost; 1: unsafe slot, Head past t
+    } else {
+      GQ_SITE(F::vacant(E) ? 2 : 3);                                  // 2: slot already at cycle >= c (invalidated); 3: occupied
+      if (!F::vacant(E)) { const int fq = (((uintptr_t)r.threshold >> 10) & 7) == 5; GQ_SITE(16 + 4 * fq + (F::cycle(E) == c ? 0 : (cycle_newer<F::kCycBits>(F::cycle(E), c) ? 1 : 2))); }
     }
     return RING_RETRY;                                                   // L163 (reading G7)
   }
@@ -300,6 +311,7 @@ struct Ring {
         return RING_OK;                                               // L182
       }
       if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
+        if (!(waited < park_ns)) GQ_SITE(F::vacant(E) ? (park_ns ? 4 : 5) : 6);   // 4: park expired, 5: no parking allowed, 6: occupied older entry
         if (waited < park_ns && F::vacant(E)) {                       // D2
           if (waited == 0 && (flags & kEagerEmpty) && counter(ld_relaxed(r.tail)) <= h) {
             park_ns = 0;                                              // polling consumers: wait only for an enqueuer that
@@ -308,7 +320,8 @@ struct Ring {
           if (thr != r.thr_reset) {                                   // D4 path, first use of thr: some dequeuer failed since
             const bool dead = thr < 0;                                // the last enqueue, so apply D1 now, with the ticket as Head
             thr = r.thr_reset;
-            if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + ((flags & kEagerEmpty) ? 0u : r.park_limit) <= h)) { park_ns = 0; continue; }
+            if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + ((flags & kEagerEmpty) ? 0u : r.park_limit) <= h)) { GQ_SITE(dead ? 7 : 8); park_ns = 0; continue; }
+            GQ_SITE(9);                                               // thr below reset seen on the D4 path, parking kept
           }
           // (Rejected, measured: sizing the nap by the place in line, h - Tail.  Any load of the hot Tail
           //  word inside the polling loop takes the ring from 37 to 12 Gops/s at k = 227 328: parked
@@ -329,6 +342,7 @@ struct Ring {
       return RING_EMPTY;
     }
     if (warp_dec<kUniform>(r.threshold) <= 0) return RING_EMPTY;      // L205-208
+    GQ_SITE(10);
     return RING_RETRY;                                                // L211
   }
 };

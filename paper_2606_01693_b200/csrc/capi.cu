@@ -515,6 +515,16 @@ static int finish_run(uint64_t* d_ctr, cudaEvent_t e0, cudaEvent_t e1, const gq_
 }
 
 // debug builds (-DGQ_DEBUG_STUCK=cap): report what the livelock detector recorded
+extern "C" int gq_dbg_sites(unsigned long long* out16) {
+#ifdef GQ_DBG_SITES
+  if (cudaMemcpyFromSymbol(out16, gq::detail::g_dbg, 32 * 8) != cudaSuccess) return -1;
+  unsigned long long z[32] = {0};
+  cudaMemcpyToSymbol(gq::detail::g_dbg, z, sizeof z);
+  return 0;
+#else
+  (void)out16; return -1;
+#endif
+}
 static void report_stuck() {
 #ifdef GQ_DEBUG_STUCK
   unsigned long long h[2 + 16 * 6];
