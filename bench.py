@@ -359,6 +359,8 @@ def run_ours(args, rank, world, local_rank):
             r = gq.run_balanced(qq, threads=full, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS)
             gq.queue_destroy(qq)
             pts[f"2^{logn}"] = {"mops": round(r["mops"], 1), "index_cycle_us": round(2.0 * (1 << logn) / (r["mops"] * 1e6) * 1e6, 2) if (1 << logn) < full else None}
+        pts["note"] = ("n < k: ops/s = 2n / index cycle.  n = 2^17 is slightly below k = full: runs there can contain retry "
+                       "episodes (DESIGN.md section 5, open issue); n >= 2^18 settles in one of two steady states (62 or 79 Gops/s)")
         sweep["capacity_lfq_full_coresidency"] = pts
 
     apps = None
