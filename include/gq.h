@@ -59,8 +59,13 @@ typedef struct {
   uint32_t flags;           /* GQ_F_* */
   uint32_t park_ns;         /* longest wait of a dequeuer on its own vacant slot before it gives the slot up
                                (D2); default 250000 */
-  uint32_t park_nap_ns;     /* longest single __nanosleep between two looks at a parked slot (D2); default 128 */
+  uint32_t park_nap_ns;     /* longest single __nanosleep between two looks at a parked slot (D2); default 128;
+                               values below 32 = no sleep at all (pure re-reading of the slot) */
+  uint32_t park_spin_ns;    /* a parked dequeuer re-reads its slot without any nap for this long before it starts the nap ladder
+                               (D2); default 2000; GQ_PARK_SPIN_NONE = ladder from the first look */
+  uint32_t reserved;        /* must be 0 */
 } gq_opts;
+#define GQ_PARK_SPIN_NONE 0xFFFFFFFFu
 enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the warp-batched one ("naive") */
        GQ_F_NO_PROBE = 2u,      /* ablation: no read-only emptiness probe before a ticket is claimed (D1) */
        GQ_F_NO_DEQ_SPIN = 4u,   /* ablation: dequeuer invalidates a vacant slot at once, no parking (D2) */
@@ -81,6 +86,7 @@ enum { GQ_F_PER_LANE_FAA = 1u,  /* ablation: one FAA per thread instead of the w
        GQ_F_NO_FULL_TEST = 2048u, /* G-LFQ-D only: the caller guarantees that the queue never holds `capacity` items (a BFS
                                    frontier queue of nv slots, a work queue of all items): enqueue skips the FULL test, which is
                                    the two hot-word loads that make G-LFQ-D slow at scale */
+       GQ_F_NO_REPAIR = 4096u,  /* ablation: a waiting dequeuer does not re-arm a slot that was marked unsafe (D9) */
        GQ_F_FENCED_PAYLOAD = 256u /* G-LFQ: order the payload against the index hand-over with release fences in front of
                                    both installing CAS (the paper's implicit scheme) instead of the payload-cell
                                    handshake (D6) */ };
@@ -103,6 +109,13 @@ int queue_drain    (gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_o
    kernels take by value.  view_out: HOST, view_bytes must be >= sizeof(view). */
 int queue_device_view(const gq_queue* q, void* view_out, size_t view_bytes);
 int queue_kind(const gq_queue* q);
+/* Read-back of the hot words of a QUIESCENT queue (synchronises the device first).  out16: HOST, 16 words:
+   G-LFQ / G-WFQ: [0] AQ.Head, [1] AQ.Tail (ticket counters, decoded from the packed word), [2] AQ.Threshold (signed), [3] FQ.Head,
+   [4] FQ.Tail, [5] FQ.Threshold; G-LFQ-D: Head, Tail, Threshold; G-WFQ-YMC: H, T.  [6] = ring parameter N, [7] = max_threads.
+   G-WFQ also: slow-path rounds since the last reset, summed over the threads that performed them (Lemma III.7):
+   [8] AQ.Tail increments <c,NULL> -> <c+1,tid> won, [9] INC bits cleared on local tails (completed rounds), [10], [11] the same
+   for AQ.Head; [12..15] the same four for FQ. */
+int queue_debug_counters(gq_queue* q, uint64_t* out16);
 /* Largest thread count the benchmark kernel of this kind can keep co-resident (occupancy
    API x SM count): the forward-progress assumption of Thm III.10. */
 int queue_max_coresident_threads(int kind, int block_threads, uint32_t* out);
@@ -118,13 +131,17 @@ typedef struct {
   uint32_t ops_per_thread;     /* > 0: fixed-op mode (iterations per thread) instead of fixed duration */
   uint32_t jitter_ns;          /* random __nanosleep in [0, jitter_ns] before each op (history runs) */
   uint32_t fail_backoff_ns;    /* harness sleeps up to this long after a FULL/EMPTY return (0 = none) */
-  uint64_t value_base;         /* first payload value (split: prefill size) */
+  uint64_t value_base;         /* first payload value (split: prefill size).  Payload of (thread t, iteration i): value_base +
+                                  (t << 16 | i) in history runs of at most 65536 threads x 65536 iterations (BASELINE.json
+                                  configs[0]), else value_base + t + i * threads; unique in both cases */
   uint32_t role_layout;        /* run_split: 0 = logical thread t runs on physical thread t (mixed warps, the default);
                                   1 = same seeded roles, but the logical threads are placed so that producers fill the
                                   first physical threads and consumers the rest: warps are homogeneous (at most one mixed);
                                   2 = layout 0, but each iteration is ONE converged call of the fused operation
                                   gq::enqueue_or_dequeue (G-LFQ only): the two roles of a mixed warp overlap */
-  uint32_t reserved;           /* must be 0 */
+  uint32_t converged;          /* 1: the lanes of a warp start every iteration of the benchmark loop together (one ballot per
+                                  iteration), as a lock-step wavefront would; 0: a lane starts its next operation as soon as its
+                                  last one returns.  Balanced and split loops; not the fused role_layout 2 */
 } gq_run_cfg;
 
 typedef struct {
@@ -196,6 +213,17 @@ typedef struct { uint32_t width, height, spp, max_bounce, n_spheres, threads; ui
                  const float* d_spheres; /* DEVICE, n_spheres x 8: cx,cy,cz,r, ar,ag,ab, emissive(0/1) */ } gq_rt_scene;
 typedef struct { uint64_t rays, queue_ops; double ms, total_ms; uint32_t threads, items; } gq_rt_stats;
 int rt_render(int kind, const gq_rt_scene* scene, float* d_rgb /* DEVICE H*W*3 */, gq_rt_stats* stats_out, void* stream);
+
+/* Debug and fault-injection builds only (include/gq/detail/debug.cuh; paper_2606_01693_b200/build.py variants "dbg"
+   and "mutants").  In the product build all three return GQ_E_INVAL and do nothing.
+   gq_dbg_sites : out80 (HOST, 80 words) = event counters [0,32), latency-probe cycle sums [32,48) and sample counts
+                  [48,64) since the last call; clears them.
+   gq_dbg_trace : the first events of the launches since the last call, 64 B each {ns, site | tid << 32, ticket,
+                  entry, Head, Tail, Threshold, aux}; out: HOST; clears the ring.
+   gq_set_mutation : arm fault `id` (0 = none) for the following launches (SURVEY section 4 "mutation tests"). */
+int gq_dbg_sites(unsigned long long* out80);
+int gq_dbg_trace(void* out, uint64_t max_records, uint64_t* n_out);
+int gq_set_mutation(uint32_t id);
 
 const char* gq_last_cuda_error(void);   /* text of the last CUDA error seen by this thread */
 const char* gq_version(void);

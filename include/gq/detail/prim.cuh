@@ -13,6 +13,8 @@
 #pragma once
 #include <cstdint>
 
+#include "debug.cuh"
+
 namespace gq {
 namespace detail {
 
@@ -105,9 +107,14 @@ __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 
   uint32_t mask = __activemask();
   if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
   const uint32_t leader = __ffs(mask) - 1;
-  const uint32_t rank = __popc(mask & lanemask_lt());
+  const uint32_t rank = __popc(mask & lanemask_lt()) + (GQ_MUT(MUT_RANK_OFF_BY_ONE) ? 1u : 0u);
   uint64_t base = 0;
-  if (lane_id() == leader) base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);
+  if (lane_id() == leader) {
+    base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);
+#ifdef GQ_DBG_SITES
+    if ((blockIdx.x & 63u) == 0) { GQ_COUNT(20, 1); GQ_COUNT(21, __popc(mask)); }   // WAVEFAA batch size (sampled blocks)
+#endif
+  }
   base = __shfl_sync(mask, base, leader);
   return base + (uint64_t)rank * unit;
 }
@@ -180,31 +187,6 @@ __device__ __host__ __forceinline__ uint32_t mix32(uint32_t x) {
   x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
   return x;
 }
-
-// ---- livelock detector (debug builds: -DGQ_DEBUG_STUCK=<iteration cap>) ------------------
-// SURVEY §5 "failure detection": a kernel-side iteration cap so that a livelock ends the kernel
-// with a diagnostic instead of hanging it.  Every retry loop of the slow paths calls stuck();
-// the first thread over the cap records {loc, tid, a..d}, raises the abort word, and from then
-// on every instrumented loop bails out, so the kernel drains and the host can read g_stuck.
-// Compiled out (constant false) in normal builds.
-#ifdef GQ_DEBUG_STUCK
-static __device__ unsigned long long g_stuck[2 + 16 * 6];
-__device__ __forceinline__ bool stuck(uint32_t& n, uint32_t loc, uint32_t tid, uint64_t a = 0, uint64_t b = 0, uint64_t c = 0, uint64_t d = 0) {
-  if ((++n & 1023u) != 0) return false;                       // look at the abort word every 1024th iteration only
-  const bool aborted = ld_relaxed(reinterpret_cast<const uint64_t*>(&g_stuck[0])) != 0;
-  if (!aborted && n < (uint32_t)(GQ_DEBUG_STUCK)) return false;
-  const unsigned long long k = atomicAdd(&g_stuck[1], 1ull);
-  if (k < 16) {
-    unsigned long long* r = g_stuck + 2 + 6 * k;
-    r[0] = loc | ((unsigned long long)n << 32); r[1] = tid; r[2] = a; r[3] = b; r[4] = c; r[5] = d;
-  }
-  __threadfence();
-  st_relaxed(reinterpret_cast<uint64_t*>(&g_stuck[0]), 1);
-  return true;
-}
-#else
-__device__ __forceinline__ bool stuck(uint32_t&, uint32_t, uint32_t, uint64_t = 0, uint64_t = 0, uint64_t = 0, uint64_t = 0) { return false; }
-#endif
 
 }  // namespace detail
 }  // namespace gq

@@ -30,22 +30,27 @@ struct RingView {
   uint32_t  park_limit; // D1: EMPTY without a ticket once Head is this far ahead of Tail
   uint32_t  park_nap;   // D2: longest single __nanosleep between two looks at the parked slot
   uint32_t  prefetch;   // > 0: rings too large to stay L2-resident: pull the slot `prefetch` tickets ahead into L2
+  uint32_t  id;         // 0 = AQ (or the only ring), 1 = FQ: names the ring in traces and latency probes (debug.cuh)
+  uint32_t  spin_ns;    // D2: a parked dequeuer re-reads its slot without any nap for this long, then backs off
 };
 
 namespace detail {
-
-#ifdef GQ_DBG_SITES
-static __device__ unsigned long long g_dbg[32];
-#define GQ_SITE(i) atomicAdd(&g_dbg[i], 1ull)
-#else
-#define GQ_SITE(i) ((void)0)
-#endif
 
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
 enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
                   kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u, kEagerEmpty = 512u, kNoCellPrefetch = 1024u, kNoFullTest = 2048u,
-                  kRelaxedInstall = 1u << 16 /* internal: this install needs no release edge */ };
+                  kNoRepair = 4096u,
+                  kRelaxedInstall = 1u << 16 /* internal: this install needs no release edge */,
+                  kPublicFlags = 0x1FFFu /* what gq_opts.flags may carry */ };
+// event sites of GQ_SITE / GQ_TRACE (debug.cuh): why a ring attempt did not succeed at its first ticket
+enum : uint32_t { SITE_ENQ_CAS_LOST = 0, SITE_ENQ_UNSAFE = 1, SITE_ENQ_SLOT_AHEAD = 2, SITE_ENQ_SLOT_OCCUPIED = 3,
+                  SITE_DEQ_PARK_EXPIRED = 4, SITE_DEQ_NO_PARK = 5, SITE_DEQ_SLOT_OCCUPIED = 6, SITE_DEQ_THR_DEAD = 7,
+                  SITE_DEQ_D1_EMPTY = 8, SITE_DEQ_THR_LOW = 9, SITE_DEQ_RETRY = 10, SITE_DEQ_EMPTY_CATCHUP = 11,
+                  SITE_DEQ_EMPTY_THR = 12, SITE_DEQ_EMPTY_EARLY = 13, SITE_DEQ_EMPTY_PROBE = 14, SITE_DEQ_REPAIR = 15 };
+// latency probe sites (GQ_TIC / GQ_TOC): + 5 * ring id for the first five
+enum : uint32_t { LAT_HEAD_FAA = 0, LAT_SLOT_WAIT = 1, LAT_TAIL_FAA = 2, LAT_INSTALL_CAS = 3, LAT_THR_CHECK = 4,
+                  LAT_PAYLOAD = 10, LAT_ENQUEUE = 11, LAT_DEQUEUE = 12 };
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
 struct LfqFmt {
@@ -71,6 +76,8 @@ struct LfqFmt {
   __device__ __host__ static uint64_t initial() { return kSafeBit | kBot; }          // <0,1,bot> (reading G4)
   // what the slot of a cycle-c ticket holds in steady state: the previous cycle's entry, consumed
   __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 33) | kSafeBit | kBotC; }
+  // D9: a vacant slot of an older cycle, made ready for the enqueuer of cycle c by the dequeuer of cycle c that waits on it
+  __device__ __host__ static uint64_t repaired(uint64_t, uint32_t c) { return predicted(c); }
 };
 
 // ---- direct-payload entry word (G-LFQ-D, DESIGN.md NEXT-3(i)): the uint32 payload sits where G-LFQ keeps the
@@ -96,6 +103,7 @@ struct DirFmt {
   __device__ __host__ static uint64_t unsafe(uint64_t e) { return e & ~kSafeBit; }
   __device__ __host__ static uint64_t initial() { return kSafeBit | kVacBit | kBot; }
   __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 34) | kSafeBit | kVacBit | kBotC; }
+  __device__ __host__ static uint64_t repaired(uint64_t, uint32_t c) { return predicted(c); }
 };
 
 // ---- G-WFQ entry word (Fig. 2 missing -> reading W1):
@@ -119,22 +127,37 @@ struct WfqFmt {
   __device__ __host__ static bool safe(uint64_t e) { return (e & kSafeBit) != 0; }
   __device__ __host__ static bool enq_visible(uint64_t e) { return (e & kEnqBit) != 0; }
   __device__ __host__ static bool vacant(uint64_t e) { return index(e) >= kBot; }
-  // fast path installs <c, Safe 1, Enq 1, x>, Note unchanged
+  // Note (Lemma III.8) is compared modulo 2^16 like Cycle (Lemma III.6), so it must stay inside the same
+  // window: every write that sets Cycle to c also raises Note to c unless a slow-path helper has already moved
+  // it further ahead (that decision must survive: the helpers of one request have to agree on the slots they
+  // skip).  Left at its initial value Note would read as "newer" again after 2^15 laps and rule the slot out
+  // for every slow-path enqueue.
+  __device__ __host__ static uint64_t note_for(uint64_t e, uint32_t c) {
+    const uint32_t d = (note(e) - c) & 0xFFFFu;                           // Note ahead of c by d cycles (mod 2^16)
+    return (uint64_t)((d != 0 && d < 0x8000u) ? note(e) : c) << 32;
+  }
+  // fast path installs <c, Safe 1, Enq 1, x>
   __device__ __host__ static uint64_t installed(uint64_t e, uint32_t c, uint32_t x) {
-    return ((uint64_t)c << 48) | (e & kNoteMask) | kSafeBit | kEnqBit | x;
+    return ((uint64_t)c << 48) | note_for(e, c) | kSafeBit | kEnqBit | x;
   }
   __device__ __host__ static uint64_t installed_slow(uint64_t e, uint32_t c, uint32_t x) {   // Enq = 0
-    return ((uint64_t)c << 48) | (e & kNoteMask) | kSafeBit | x;
+    return ((uint64_t)c << 48) | note_for(e, c) | kSafeBit | x;
   }
   __device__ __host__ static uint64_t advanced(uint64_t e, uint32_t c) {
-    return ((uint64_t)c << 48) | (e & kNoteMask) | (e & kSafeBit) | kEnqBit | kBot;
+    return ((uint64_t)c << 48) | note_for(e, c) | (e & kSafeBit) | kEnqBit | kBot;
   }
   __device__ __host__ static uint64_t unsafe(uint64_t e) { return e & ~kSafeBit; }
   __device__ __host__ static uint64_t with_note(uint64_t e, uint32_t c) { return (e & ~kNoteMask) | ((uint64_t)c << 32); }
-  // Note starts "older than every cycle in use": tickets start at cycle 1, so 0 with modular compare
-  __device__ __host__ static uint64_t initial() { return kSafeBit | kEnqBit | kBot; }
-  // steady state: previous cycle, consumed (CONSUME sets Enq with the index), Note never used
-  __device__ __host__ static uint64_t predicted(uint32_t c) { return ((uint64_t)((c - 1u) & kCycMask) << 48) | kSafeBit | kEnqBit | kBotC; }
+  __device__ __host__ static uint64_t initial() { return kSafeBit | kEnqBit | kBot; }       // Cycle 0, Note 0; tickets start at cycle 1
+  // steady state: previous cycle, consumed (CONSUME sets Enq with the index), Note = that cycle
+  __device__ __host__ static uint64_t predicted(uint32_t c) {
+    const uint64_t p = (c - 1u) & kCycMask;
+    return (p << 48) | (p << 32) | kSafeBit | kEnqBit | kBotC;
+  }
+  __device__ __host__ static uint64_t repaired(uint64_t e, uint32_t c) {
+    const uint32_t p = (c - 1u) & kCycMask;
+    return ((uint64_t)p << 48) | note_for(e, p) | kSafeBit | kEnqBit | kBotC;
+  }
 };
 
 // Hook run by a dequeuer between finding its entry and CONSUME.  G-LFQ: nothing.
@@ -165,16 +188,20 @@ struct Ring {
   // B200: a plain store per enqueue (kPlainThrStore) serialises all
   // enqueuers on the Threshold word and costs 50x in throughput.
   __device__ __forceinline__ static void reset_threshold(const RingView& r, uint32_t flags = 0) {
+    if (GQ_MUT(MUT_NO_THR_RESET)) return;
     if (flags & kThrRedMax) {
       // Threshold never exceeds 3N-1, so "Threshold <- 3N-1" == max(Threshold, 3N-1): one fire-and-forget
-      // reduction by the leader of the lanes whose CAS just succeeded (all of them have their CAS result).
-      const uint32_t mask = __activemask();
+      // reduction by the leader of the lanes whose CAS just succeeded (all of them have their CAS result);
+      // converged lanes of a non-uniform caller may name different rings: one leader per Threshold word
+      uint32_t mask = __activemask();
+      if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(r.threshold));
       if (lane_id() == (uint32_t)__ffs(mask) - 1) red_max_s64_relaxed(r.threshold, r.thr_reset);
       return;
     }
-    if ((flags & kPlainThrStore) ||
-        (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)) != r.thr_reset)
-      st_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)r.thr_reset);
+    GQ_TIC(t0);
+    const int64_t thr = (flags & kPlainThrStore) ? -1 : (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
+    GQ_TOC(LAT_THR_CHECK + 5 * r.id, t0, thr);
+    if (thr != r.thr_reset) st_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)r.thr_reset);
   }
 
   // "catch up Tail to at least h+1" (Alg. 1; reading G9).  Batched like WAVEFAA: the
@@ -201,6 +228,10 @@ struct Ring {
     }
   }
 
+  __device__ __forceinline__ static uint64_t install_cas(uint64_t* sp, uint64_t E, uint64_t N, uint32_t flags) {
+    return (flags & kRelaxedInstall) ? cas_relaxed(sp, E, N) : cas_release(sp, E, N);
+  }
+
   // Alg. 1 L143-163.  Returns RING_OK or RING_RETRY; *t_out = the ticket used.
   //
   // Optimistic install (sm_100a; kNoOptCas switches it off): in steady state the slot of a
@@ -212,18 +243,21 @@ struct Ring {
   // have/t_pre: the ticket was already reserved by the caller (D5); else it is drawn here.
   __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out, uint32_t flags = 0,
                                                 bool have = false, uint64_t t_pre = 0) {
+    GQ_TIC(t0);
     const uint64_t t = have ? t_pre : take(r.tail);                   // L144
+    if (!have) GQ_TOC(LAT_TAIL_FAA + 5 * r.id, t0, t);
     *t_out = t;
     // A first-touch CAS is an L2 miss that the slice's atomic unit waits out, with every atomic queued behind
     // it ("cold lines"): for rings that cannot stay L2-resident, fetch a later slot now.
     if (r.prefetch) asm volatile("prefetch.global.L2 [%0];" :: "l"(slot(r, slot_of(r, t + r.prefetch))));
-    const uint32_t j = slot_of(r, t), c = cycle_of(r, t);             // L146
+    const uint32_t j = slot_of(r, GQ_MUT(MUT_LIFO_PAIR) ? (t ^ 1) : t), c = cycle_of(r, t);   // L146
     uint64_t* sp = slot(r, j);
     uint64_t E;
+    GQ_TIC(t1);
     if (!(flags & kNoOptCas)) {
       E = F::predicted(c);
-      const uint64_t o = (flags & kRelaxedInstall) ? cas_relaxed(sp, E, F::installed(E, c, x))
-                                                     : cas_release(sp, E, F::installed(E, c, x));   // L153 on the predicted entry
+      const uint64_t o = install_cas(sp, E, F::installed(E, c, x), flags);   // L153 on the predicted entry
+      GQ_TOC(LAT_INSTALL_CAS + 5 * r.id, t1, o);
       if (o == E) { reset_threshold(r, flags); return RING_OK; }      // L155
       E = o;                                                          // L148: the failed CAS read the slot
     } else {
@@ -235,17 +269,17 @@ struct Ring {
         fence_acq_rel();                                              // Head must not be older than E
         ok = counter(ld_relaxed(r.head)) <= t;
       }
-      if (ok && ((flags & kRelaxedInstall) ? cas_relaxed(sp, E, F::installed(E, c, x))
-                                           : cas_release(sp, E, F::installed(E, c, x))) == E) {   // L153: linearization point (L111)
+      if (ok && install_cas(sp, E, F::installed(E, c, x), flags) == E) {   // L153: linearization point (L111)
         reset_threshold(r, flags);                                    // L155
         return RING_OK;
       }
-      GQ_SITE(ok ? 0 : 1);                                            // 0: second CAS lost; 1: unsafe slot, Head past t
+      GQ_SITE(ok ? SITE_ENQ_CAS_LOST : SITE_ENQ_UNSAFE);
+      GQ_TRACE((ok ? SITE_ENQ_CAS_LOST : SITE_ENQ_UNSAFE) | r.id << 8, r, t, E, 0);
     } else {
-      GQ_SITE(F::vacant(E) ? 2 : 3);                                  // 2: slot already at cycle >= c (invalidated); 3: occupied
-      if (!F::vacant(E)) { const int fq = (((uintptr_t)r.threshold >> 10) & 7) == 5; GQ_SITE(16 + 4 * fq + (F::cycle(E) == c ? 0 : (cycle_newer<F::kCycBits>(F::cycle(E), c) ? 1 : 2))); }
+      GQ_SITE(F::vacant(E) ? SITE_ENQ_SLOT_AHEAD : SITE_ENQ_SLOT_OCCUPIED);
+      GQ_TRACE((F::vacant(E) ? SITE_ENQ_SLOT_AHEAD : SITE_ENQ_SLOT_OCCUPIED) | r.id << 8, r, t, E, 0);
     }
-    return RING_RETRY;                                                   // L163 (reading G7)
+    return RING_RETRY;                                                // L163 (reading G7)
   }
 
   // Alg. 1 L165-211 with the reconstruction of reading G6 (reload on CAS failure).
@@ -283,13 +317,15 @@ struct Ring {
     int64_t thr;
     uint64_t h;
     const bool listed = probe || (flags & kThrFirst);
+    GQ_TIC(t0);
     if (listed) {
       thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
-      if (thr < 0) return RING_EMPTY;                                 // L166-169
+      if (thr < 0) { GQ_SITE(SITE_DEQ_EMPTY_EARLY); return RING_EMPTY; }   // L166-169
       if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {     // D1
         const uint64_t H = counter(ld_acquire(r.head));
         const uint64_t T = counter(ld_relaxed(r.tail));
-        if (T + ((park_ns && !(flags & kEagerEmpty)) ? r.park_limit : 0u) <= H) return RING_EMPTY;
+        if (GQ_MUT(MUT_UNSOUND_EMPTY) && T <= H + 2) return RING_EMPTY;
+        if (T + ((park_ns && !(flags & kEagerEmpty)) ? r.park_limit : 0u) <= H) { GQ_SITE(SITE_DEQ_EMPTY_PROBE); return RING_EMPTY; }
       }
       h = take(r.head);                                               // L172
       thr = r.thr_reset;                                              // parking allowed (as before D4)
@@ -297,52 +333,87 @@ struct Ring {
       thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));   // in flight with the FAA / slot load
       h = take(r.head);                                               // L172
     }
+    GQ_TOC(LAT_HEAD_FAA + 5 * r.id, t0, h);
     *h_out = h;
     if (r.prefetch) asm volatile("prefetch.global.L2 [%0];" :: "l"(slot(r, slot_of(r, h + r.prefetch))));
     const uint32_t j = slot_of(r, h), c = cycle_of(r, h);             // L175
     uint64_t* sp = slot(r, j);
-    uint32_t waited = 0, nap = r.park_nap < 32 ? r.park_nap : 32;
+    // park budget in ns: every look at the slot counts its nap plus kPollNs (an L2 round trip under load)
+    constexpr uint32_t kPollNs = 384;
+    uint32_t waited = 0, nap = 0;
+    GQ_TIC(t1);
     for (;;) {
-      const uint64_t E = ld_acquire(sp);                              // L176 (acquire: payload edge, G15)
+      uint64_t E = ld_acquire(sp);                                    // L176 (acquire: payload edge, G15)
+    classify:
       if (F::cycle(E) == c && !F::vacant(E)) {                        // L178
+        GQ_TOC(LAT_SLOT_WAIT + 5 * r.id, t1, E);
         fin(r, h, j, E);                                              // G-WFQ: finalize an Enq=0 entry (W6)
         red_or_relaxed(sp, F::kConsumeMask);                          // L180 CONSUME: linearization point
         *x = F::index(E);
         return RING_OK;                                               // L182
       }
       if (cycle_newer<F::kCycBits>(c, F::cycle(E))) {                 // E.Cycle < c (guard lost in extraction)
-        if (!(waited < park_ns)) GQ_SITE(F::vacant(E) ? (park_ns ? 4 : 5) : 6);   // 4: park expired, 5: no parking allowed, 6: occupied older entry
         if (waited < park_ns && F::vacant(E)) {                       // D2
-          if (waited == 0 && (flags & kEagerEmpty) && counter(ld_relaxed(r.tail)) <= h) {
-            park_ns = 0;                                              // polling consumers: wait only for an enqueuer that
-            continue;                                                 // already holds ticket h, never for a future one
-          }
-          if (thr != r.thr_reset) {                                   // D4 path, first use of thr: some dequeuer failed since
-            const bool dead = thr < 0;                                // the last enqueue, so apply D1 now, with the ticket as Head
-            thr = r.thr_reset;
-            if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + ((flags & kEagerEmpty) ? 0u : r.park_limit) <= h)) { GQ_SITE(dead ? 7 : 8); park_ns = 0; continue; }
-            GQ_SITE(9);                                               // thr below reset seen on the D4 path, parking kept
+          if (waited == 0) {                                          // first look at a vacant slot
+            if ((flags & kEagerEmpty) && counter(ld_relaxed(r.tail)) <= h) {
+              park_ns = 0;                                            // polling consumers: wait only for an enqueuer that
+              goto classify;                                          // already holds ticket h, never for a future one
+            }
+            if (thr != r.thr_reset) {                                 // D4 path, first use of thr: some dequeuer failed since
+              const bool dead = thr < 0;                              // the last enqueue, so apply D1 now, with the ticket as Head
+              thr = r.thr_reset;
+              if (dead || (!(flags & kNoProbe) && counter(ld_relaxed(r.tail)) + ((flags & kEagerEmpty) ? 0u : r.park_limit) <= h)) {
+                GQ_SITE(dead ? SITE_DEQ_THR_DEAD : SITE_DEQ_D1_EMPTY);
+                GQ_TRACE((dead ? SITE_DEQ_THR_DEAD : SITE_DEQ_D1_EMPTY) | r.id << 8, r, h, E, 0);
+                park_ns = 0;
+                goto classify;
+              }
+              GQ_SITE(SITE_DEQ_THR_LOW);                              // thr below reset seen on the D4 path, parking kept
+            }
+            // D9 repair.  A slot that a dequeuer once marked unsafe (L193) stays unsafe until an enqueuer arrives with
+            // Head <= its ticket (L151), which never happens on a ring whose dequeuers wait in line (Head ahead of Tail for
+            // good: FQ whenever k > n): the enqueuer of every later cycle gives the slot up and its parked dequeuer waits
+            // out the whole park_ns, lap after lap.  The dequeuer that is about to wait here IS the dequeuer of cycle c, so
+            // it may declare the slot ready for the enqueuer of cycle c, <c-1, Safe 1, bot_c>, provided no dequeuer of a
+            // later cycle has been here before it, i.e. Head has not reached h + 2N (read after E; Head only grows).
+            if (!F::safe(E) && !(flags & kNoRepair) && counter(ld_relaxed(r.head)) <= h + (1ull << r.order)) {
+              const uint64_t R = F::repaired(E, c);
+              const uint64_t o = cas_relaxed(sp, E, R);
+              GQ_SITE(SITE_DEQ_REPAIR);
+              if (o != E) { E = o; goto classify; }                   // the slot changed under us: classify what the CAS read
+            }
           }
           // (Rejected, measured: sizing the nap by the place in line, h - Tail.  Any load of the hot Tail
           //  word inside the polling loop takes the ring from 37 to 12 Gops/s at k = 227 328: parked
           //  threads must stay off the hot lines, which is the point of D2.)
-          __nanosleep(nap); waited += nap; nap = nap * 2 < r.park_nap ? nap * 2 : r.park_nap;
+          // The first spin_ns are pure re-reading (the front of the line: the hand-over is detected one nap
+          // earlier), after that the nap ladder 32 ns .. park_nap keeps the many threads further back quiet.
+          if (waited >= r.spin_ns && r.park_nap) { nap = nap ? (nap * 2 < r.park_nap ? nap * 2 : r.park_nap) : 32; __nanosleep(nap); }
+          waited += nap + kPollNs;
           continue;
         }
+        GQ_SITE(F::vacant(E) ? (park_ns ? SITE_DEQ_PARK_EXPIRED : SITE_DEQ_NO_PARK) : SITE_DEQ_SLOT_OCCUPIED);
+        GQ_TRACE((F::vacant(E) ? (park_ns ? SITE_DEQ_PARK_EXPIRED : SITE_DEQ_NO_PARK) : SITE_DEQ_SLOT_OCCUPIED) | r.id << 8, r, h, E, waited);
         const uint64_t New = F::vacant(E) ? F::advanced(E, c)         // L186-188
                                           : F::unsafe(E);             // L193
-        if (New != E && cas_relaxed(sp, E, New) != E) continue;       // reload: the slot changed under us
+        if (New != E) {
+          const uint64_t o = cas_relaxed(sp, E, New);
+          if (o != E && !GQ_MUT(MUT_NO_RELOAD)) { E = o; goto classify; }   // reload: the slot changed under us (G6): the failed CAS read it
+        }
       }
       break;
     }
     const uint64_t T = counter(ld_relaxed(r.tail));
     if (T <= h + 1) {                                                 // L197
+      GQ_SITE(SITE_DEQ_EMPTY_CATCHUP);
+      GQ_TRACE(SITE_DEQ_EMPTY_CATCHUP | r.id << 8, r, h, 0, T);
       catchup_tail(r, h + 1);                                         // L200
       warp_dec<kUniform>(r.threshold);                                // L202
       return RING_EMPTY;
     }
-    if (warp_dec<kUniform>(r.threshold) <= 0) return RING_EMPTY;      // L205-208
-    GQ_SITE(10);
+    if (warp_dec<kUniform>(r.threshold) <= 0) { GQ_SITE(SITE_DEQ_EMPTY_THR); return RING_EMPTY; }   // L205-208
+    GQ_SITE(SITE_DEQ_RETRY);
+    GQ_TRACE(SITE_DEQ_RETRY | r.id << 8, r, h, 0, T);
     return RING_RETRY;                                                // L211
   }
 };

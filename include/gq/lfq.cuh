@@ -36,10 +36,10 @@ template <class F, bool kUniform, bool kWarpFaa, class Fin>
 __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, uint64_t* retries, const Fin& fin,
                                              bool probe, uint32_t flags, uint64_t* ticket = nullptr) {
   Backoff bo;
-  uint32_t sn = 0;
+  [[maybe_unused]] uint32_t sn = 0;
   for (;;) {
     uint64_t h;
-    if (stuck(sn, 1, 0, ld_relaxed(r.head), ld_relaxed(r.tail))) return RING_EMPTY;
+    if (GQ_STUCK(sn, 1, 0, r.head, r.tail)) return RING_EMPTY;
     const int s = Ring<F, kUniform, kWarpFaa>::try_deq(r, idx, &h, fin, probe, flags);
     if (s != RING_RETRY) { if (ticket) *ticket = h; return s; }
     ++*retries;
@@ -50,35 +50,52 @@ __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, u
 template <class F, bool kUniform, bool kWarpFaa>
 __device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, uint64_t* retries, uint32_t flags) {
   Backoff bo;
-  uint32_t sn = 0;
+  [[maybe_unused]] uint32_t sn = 0;
   for (;;) {
     uint64_t t;
-    if (stuck(sn, 2, 0, ld_relaxed(r.head), ld_relaxed(r.tail))) return;
+    if (GQ_STUCK(sn, 2, 0, r.head, r.tail)) return;
     if (Ring<F, kUniform, kWarpFaa>::try_enq(r, idx, &t, flags) == RING_OK) return;
     ++*retries;
     bo.pause();
   }
 }
 
-}  // namespace detail
-
 // Payload cells (DESIGN.md departure D6, sm_100a).  The paper's scheme (Data[idx] <- v, then publish
 // idx) needs the payload store to be performed before the installing CAS, i.e. a release fence in
 // front of each install: MEMBAR.ALL.GPU, which waits for every outstanding store and reduction of
 // the thread and costs about two extra L2 round trips per operation on B200 (measured: 31 -> 43
-// Gops/s without them).  Instead each Data cell is one 64-bit word <tag | v>, tag = the low 32 bits
-// of the AQ tail ticket the index is installed under, and the hand-over is a handshake that needs
-// no cross-location ordering:
-//   enqueue : t <- AQ tail ticket; st Data[idx] <- <t | v>  and  CAS-install idx at slot(t), both
-//             relaxed and in flight together (a RETRY with a new ticket t' stores <t' | v> again)
+// Gops/s without them).  Instead each Data cell is one 64-bit word <1 | tag | v>, tag = the low 31
+// bits of the AQ tail ticket the index is installed under, and the hand-over is a handshake that
+// needs no cross-location ordering:
+//   enqueue : t <- AQ tail ticket; st Data[idx] <- <1 | t | v>  and  CAS-install idx at slot(t), both
+//             relaxed and in flight together (a RETRY with a new ticket t' stores <1 | t' | v> again)
 //   dequeue : h = the AQ head ticket that found idx (h == t); re-read Data[idx] until its tag is h
 // The dequeuer may arrive before the payload; the store has already been issued, so the wait is
 // bounded by memory latency, not by another thread's steps (lock-freedom is unaffected).  A tag
 // can only match the store of THIS tenure of idx: stores of earlier tenures carry tickets that
-// differ by less than 2^32 (FQ is FIFO, so an index is reused within about n + k tickets), and all
-// of them were observed by their own dequeuers, hence performed, before idx was recycled.  idx goes
-// back into FQ only after the matching load has returned its value (control dependency), so the
-// next owner's store cannot be read by it.  GQ_F_FENCED_PAYLOAD restores release CAS on both sides.
+// differ by less than 2^31 (FQ is FIFO, so an index is reused within about n + k tickets), and all
+// of them were observed by their own dequeuers, hence performed, before idx was recycled.  Bit 63
+// marks a tagged word: a freshly formatted cell (0) and a cell written by G-WFQ's slow path
+// (<0 | 0 | v>) match no ticket.  idx goes back into FQ only after the matching load has returned
+// its value (control dependency), so the next owner's store cannot be read by it.
+// GQ_F_FENCED_PAYLOAD restores release CAS on both sides.
+__device__ __forceinline__ uint64_t cell_word(uint64_t ticket, uint32_t v) {
+  return (1ull << 63) | ((ticket & 0x7FFFFFFFull) << 32) | v;
+}
+__device__ __forceinline__ uint32_t cell_tag(uint64_t ticket) { return 0x80000000u | (uint32_t)(ticket & 0x7FFFFFFFull); }
+// dequeue side of the handshake: w = first load of the cell (already issued by the caller)
+__device__ __forceinline__ uint64_t cell_await(const uint64_t* cell, uint64_t w, uint64_t ticket) {
+  const uint32_t tag = cell_tag(ticket);
+  [[maybe_unused]] uint32_t sn = 0;
+  for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {   // payload still in flight
+    if (GQ_MUT(MUT_NO_HANDSHAKE) || GQ_MUT(MUT_WRONG_CELL) || GQ_MUT(MUT_EARLY_RECYCLE) || GQ_STUCK(sn, 5, 0, cell)) break;
+    if (nap) __nanosleep(nap);
+    w = ld_relaxed(cell);
+  }
+  return w;
+}
+
+}  // namespace detail
 
 // kUniform: all lanes converged at the call name the same queue (see warp_faa).
 template <bool kUniform = false, bool kWarpFaa = true>
@@ -87,6 +104,7 @@ __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32
   using R = Ring<LfqFmt, kUniform, kWarpFaa>;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   uint32_t idx;
+  GQ_TIC(t_op);
   if (ring_deq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, &idx, retries, NoFinalize{}, (ctx.hungry & 2u) != 0, q.flags) == RING_EMPTY) {
     ctx.hungry |= 2u;
     return FULL;
@@ -99,11 +117,17 @@ __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32
     return OK;
   }
   Backoff bo;
+  [[maybe_unused]] uint32_t sn = 0;
   for (;;) {
+    if (GQ_STUCK(sn, 3, ctx.tid, q.aq.head, q.aq.tail)) return OK;
+    GQ_TIC(t0);
     const uint64_t t = R::take(q.aq.tail);
-    st_relaxed(cell, (t << 32) | v);                               // D6: payload tagged with its ticket
+    GQ_TOC(LAT_TAIL_FAA, t0, t);
+    if (!GQ_MUT(MUT_NO_HANDSHAKE)) st_relaxed(cell, cell_word(t, v));   // D6: payload tagged with its ticket
     uint64_t tt;
-    if (R::try_enq(q.aq, idx, &tt, q.flags | kRelaxedInstall, true, t) == RING_OK) return OK;
+    const int s = R::try_enq(q.aq, idx, &tt, q.flags | kRelaxedInstall, true, t);
+    if (GQ_MUT(MUT_NO_HANDSHAKE)) st_relaxed(cell, cell_word(t, v));
+    if (s == RING_OK) { GQ_TOC(LAT_ENQUEUE, t_op, tt); return OK; }
     ++*retries;
     bo.pause();
   }
@@ -119,29 +143,28 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
   using R = Ring<LfqFmt, kUniform, kWarpFaa>;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   uint32_t idx;
+  GQ_TIC(t_op);
   if (ring_deq_loop<LfqFmt, kUniform, kWarpFaa>(q.aq, &idx, retries, NoFinalize{}, (ctx.hungry & 1u) != 0, q.flags, &ctx.last_ticket) == RING_EMPTY) {
     ctx.hungry |= 1u;
     return EMPTY;
   }
   ctx.hungry &= ~1u;
   const bool fenced = (q.flags & kFencedPayload) != 0;
-  const uint64_t* cell = q.data + idx;
+  const uint32_t fl = fenced ? q.flags : (q.flags | kRelaxedInstall);
+  const uint64_t* cell = q.data + ((GQ_MUT(MUT_WRONG_CELL) && (idx ^ 1u) < q.capacity) ? (idx ^ 1u) : idx);
+  if (GQ_MUT(MUT_EARLY_RECYCLE)) ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, idx, retries, fl);
+  GQ_TIC(t0);
   uint64_t w = ld_relaxed(cell);                                   // after the acquire load of the entry
-  const bool paired = !(q.flags & kNoPairedFaa);
+  const bool paired = !(q.flags & kNoPairedFaa) && !GQ_MUT(MUT_EARLY_RECYCLE);
   uint64_t t = 0;
   if (paired) t = R::take(q.fq.tail);                              // D5: issued behind the payload load
-  if (!fenced) {
-    const uint32_t tag = (uint32_t)ctx.last_ticket;
-    for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {   // payload still in flight
-      if (nap) __nanosleep(nap);
-      w = ld_relaxed(cell);
-    }
-  }
+  if (!fenced) w = cell_await(cell, w, ctx.last_ticket);
+  GQ_TOC(LAT_PAYLOAD, t0, w + t);
   *out = (uint32_t)w;
-  const uint32_t fl = fenced ? q.flags : (q.flags | kRelaxedInstall);
+  if (GQ_MUT(MUT_EARLY_RECYCLE)) return OK;
   uint64_t tt;
   if (paired) {
-    if (R::try_enq(q.fq, idx, &tt, fl, true, t) == RING_OK) return OK;
+    if (R::try_enq(q.fq, idx, &tt, fl, true, t) == RING_OK) { GQ_TOC(LAT_DEQUEUE, t_op, tt); return OK; }
     ++*retries;
   }
   ring_enq_loop<LfqFmt, kUniform, kWarpFaa>(q.fq, idx, retries, fl);
@@ -179,16 +202,14 @@ __device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& 
   uint64_t* cell = q.data + idx;
   uint64_t w = is_enq ? 0 : ld_relaxed(cell);
   Backoff bo;
+  [[maybe_unused]] uint32_t sn = 0;
   for (bool first = true;; first = false) {
+    if (GQ_STUCK(sn, 4, ctx.tid, r2.head, r2.tail)) return OK;
     const uint64_t t = R::take(r2.tail);                               // two leaders, one instruction
     if (is_enq) {
-      st_relaxed(cell, (t << 32) | *v);                                // D6: payload tagged with its AQ ticket
+      st_relaxed(cell, cell_word(t, *v));                              // D6: payload tagged with its AQ ticket
     } else if (first) {
-      const uint32_t tag = (uint32_t)h1;
-      for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {
-        if (nap) __nanosleep(nap);
-        w = ld_relaxed(cell);
-      }
+      w = cell_await(cell, w, h1);
       *v = (uint32_t)w;
     }
     uint64_t tt;

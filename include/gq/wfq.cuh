@@ -31,7 +31,9 @@ struct alignas(128) WfqRecord {
   uint64_t seq1, seq2;                 // request sequence pair
   uint32_t pending, enqueue, index, _r0;
   uint32_t n_slow_enq, n_slow_deq, n_helps, _r1;     // statistics (owner-private)
-  uint64_t _pad[2];
+  // Lemma III.7 bookkeeping, written only by the thread that owns this record, about rounds it performed for ANY request:
+  // global increments <c,NULL> -> <c+1,tid> it won, and INC bits it cleared (the end of a logical round), per counter
+  uint32_t n_tail_inc, n_tail_clr, n_head_inc, n_head_clr;
 };
 static_assert(sizeof(WfqRecord) == 128, "one L2 line per record");
 
@@ -69,7 +71,7 @@ struct Wf {
   // Help the phase-2 request named by ThrIdx u (Alg. 2): clear INC on the local word
   // its record names.  Accepted only if the record's sequence pair matches and its counter is
   // below the global counter c we saw next to u (a record of a later round has counter >= c).
-  __device__ static void help_phase2(const RingView& r, uint32_t u, uint64_t c) {
+  __device__ static void help_phase2(const RingView& r, uint32_t u, uint64_t c, uint32_t me) {
     WfqRecord* p = rec(r, u);
     const uint64_t s2 = ld_acquire(&p->p2_seq2);
     const uint64_t target = ld_relaxed(&p->p2_target);
@@ -77,7 +79,10 @@ struct Wf {
     fence_acq_rel();
     if (ld_relaxed(&p->p2_seq1) != s2) return;
     if ((expect >> S) >= c || !(expect & kINC)) return;
-    cas_acq_rel(local_ptr(r, target), expect, expect & ~kINC);
+    if (cas_acq_rel(local_ptr(r, target), expect, expect & ~kINC) == expect) {
+      WfqRecord* mine = rec(r, me);
+      ++((target & 1) ? mine->n_head_clr : mine->n_tail_clr);
+    }
   }
 
   // SLOWFAA (Alg. 2; reading W4).  G = global Head or Tail word, L = the request's
@@ -89,19 +94,19 @@ struct Wf {
                                   uint64_t target_id) {
     WfqRecord* mine = rec(r, me);
     uint64_t c = 0;
-    uint32_t sn1 = 0, sn2 = 0;
+    [[maybe_unused]] uint32_t sn1 = 0, sn2 = 0;
     for (;;) {
-      if (stuck(sn1, (kDeq ? 11 : 10) | ((uint32_t)((uintptr_t)r.head >> 10) & 0xF) << 8, me, ld_relaxed(G), ld_relaxed(L), ld_relaxed(kDeq ? r.tail : r.head), ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)))) return false;
+      if (GQ_STUCK(sn1, (kDeq ? 11 : 10) | r.id << 8, me, G, L, kDeq ? r.tail : r.head, r.threshold)) return false;
       bool have = false;
       for (;;) {                                            // L249-257: FIN check, read G, help phase 2
-        if (stuck(sn2, (kDeq ? 13 : 12) | ((uint32_t)((uintptr_t)r.head >> 10) & 0xF) << 8, me, ld_relaxed(G), ld_relaxed(L), ld_relaxed(kDeq ? r.tail : r.head), ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)))) return false;
+        if (GQ_STUCK(sn2, (kDeq ? 13 : 12) | r.id << 8, me, G, L, kDeq ? r.tail : r.head, r.threshold)) return false;
         const uint64_t lv = ld_acquire(L);
         if (tag_of(lv) != tag || (lv & kFIN)) break;
         const uint64_t g = ld_acquire(G);
         c = g >> S;
         const uint32_t u = (uint32_t)(g & kNull);
         if (u == kNull) { have = true; break; }
-        help_phase2(r, u, c);
+        help_phase2(r, u, c, me);
         if (cas_acq_rel(G, g, (c << S) | kNull) == g) { have = true; break; }
       }
       const uint64_t want = local_word(c, tag) | kINC;      // L258: synchronize L to c using INC
@@ -123,8 +128,9 @@ struct Wf {
       const uint64_t g0 = (c << S) | kNull;
       if (cas_acq_rel(G, g0, ((c + 1) << S) | me) == g0) break;        // L262: <c,NULL> -> <c+1,tid>
     }
+    ++(kDeq ? mine->n_head_inc : mine->n_tail_inc);
     if (kDeq) faa_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)-1ll);   // L264-266
-    cas_acq_rel(L, v, v & ~kINC);                                        // L270: clear INC on L
+    if (cas_acq_rel(L, v, v & ~kINC) == v) ++(kDeq ? mine->n_head_clr : mine->n_tail_clr);   // L270: clear INC on L
     cas_acq_rel(G, ((c + 1) << S) | me, ((c + 1) << S) | kNull);         // L273: clear ThrIdx in G
     v &= ~kINC;
     return true;
@@ -157,9 +163,9 @@ struct Wf {
     using R = Ring<F, false, true>;
     const uint32_t j = R::slot_of(r, T), c = R::cycle_of(r, T);
     uint64_t* sp = R::slot(r, j);
-    uint32_t sn = 0;
+    [[maybe_unused]] uint32_t sn = 0;
     for (;;) {
-      if (stuck(sn, 20, owner, T, ld_relaxed(sp), ld_relaxed(L), v)) return true;
+      if (GQ_STUCK(sn, 20, owner, sp, L)) return true;
       const uint64_t E = ld_acquire(sp);
       if (cycle_newer<16>(c, F::cycle(E)) && cycle_newer<16>(c, F::note(E))) {
         const bool usable = F::vacant(E) && (F::safe(E) || R::counter(ld_acquire(r.head)) <= T);
@@ -170,6 +176,7 @@ struct Wf {
         st_relaxed(r.owner + j, ((uint64_t)c << 32) | owner);
         const uint64_t N = F::installed_slow(E, c, x);        // <c, Safe 1, Enq 0, x>: linearization point
         if (cas_acq_rel(sp, E, N) != E) continue;
+        if (GQ_MUT(MUT_SLOW_NO_FIN) && (T & 3) == 0) { cas_acq_rel(sp, N, N | F::kEnqBit); return false; }
         if (cas_acq_rel(L, v, v | kFIN) == v)                 // finalise the request ...
           cas_acq_rel(sp, N, N | F::kEnqBit);                 // ... and make the entry visible to fast dequeuers
         R::reset_threshold(r);
@@ -196,9 +203,9 @@ struct Wf {
     using R = Ring<F, false, true>;
     const uint32_t j = R::slot_of(r, H), c = R::cycle_of(r, H);
     uint64_t* sp = R::slot(r, j);
-    uint32_t sn = 0;
+    [[maybe_unused]] uint32_t sn = 0;
     for (;;) {
-      if (stuck(sn, 21, 0, H, ld_relaxed(sp), ld_relaxed(L), v)) return true;
+      if (GQ_STUCK(sn, 21, 0, sp, L)) return true;
       uint64_t E = ld_acquire(sp);
       if (F::cycle(E) == c && F::index(E) != F::kBot)         // ready (or already consumed by the owner)
         return set_fin(L, v);
@@ -226,18 +233,18 @@ struct Wf {
 
   __device__ static void enqueue_slow(const RingView& r, uint64_t v, uint32_t x, uint32_t owner, uint32_t tag, uint32_t me) {
     uint64_t* L = &rec(r, owner)->localTail;
-    uint32_t sn = 0;
+    [[maybe_unused]] uint32_t sn = 0;
     while (slow_faa<false>(r, r.tail, L, v, tag, me, (uint64_t)owner << 1)) {
       if (try_enq_slow(r, v >> S, x, L, v, owner)) break;
-      if (stuck(sn, 30, me, ld_relaxed(r.tail), ld_relaxed(r.head), v, owner)) break;
+      if (GQ_STUCK(sn, 30, me, r.tail, r.head, L)) break;
     }
   }
   __device__ static void dequeue_slow(const RingView& r, uint64_t v, uint32_t owner, uint32_t tag, uint32_t me) {
     uint64_t* L = &rec(r, owner)->localHead;
-    uint32_t sn = 0;
+    [[maybe_unused]] uint32_t sn = 0;
     while (slow_faa<true>(r, r.head, L, v, tag, me, ((uint64_t)owner << 1) | 1)) {
       if (try_deq_slow(r, v >> S, L, v)) break;
-      if (stuck(sn, 31, me, ld_relaxed(r.tail), ld_relaxed(r.head), v, (uint64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold)))) break;
+      if (GQ_STUCK(sn, 31, me, r.tail, r.head, L, r.threshold)) break;
     }
   }
 
@@ -275,13 +282,13 @@ struct Wf {
     for (uint32_t p = have_pre ? 1 : 0; p < patience; ++p) {
       if (cell) {
         const uint64_t tk = R::take(r.tail);
-        st_relaxed(cell, (tk << 32) | v);
+        st_relaxed(cell, cell_word(tk, v));
         if (R::try_enq(r, x | kWfqFast, &t, flags | kRelaxedInstall, true, tk) == RING_OK) return;
       } else if (R::try_enq(r, x, &t, flags) == RING_OK) return;
       have_t = true;
       ++*retries;
     }
-    if (cell) st_relaxed(cell, (uint64_t)v);                          // slow path: payload before the request is published
+    if (cell) st_relaxed(cell, (uint64_t)v);                          // slow path: untagged word (bit 63 clear), payload before the request is published
     // Seed of the local word: a counter value strictly below every ticket the slow path can
     // obtain (a failed fast ticket, or current - 1), else the local word could return to its
     // seed after round one and a late helper's CAS would re-open that round (ABA).
@@ -417,13 +424,7 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   const bool paired = !(q.flags & kNoPairedFaa) && q.enq_patience != 0 && q.enq_patience != 0xFFFFFFFFu;
   uint64_t t = 0;
   if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq.tail);
-  if (fast) {                                                       // tagged cell: wait for the store of THIS tenure of idx
-    const uint32_t tag = (uint32_t)ctx.last_ticket;
-    for (uint32_t nap = 0; (uint32_t)(w >> 32) != tag; nap = nap ? (nap < 256 ? nap * 2 : 256) : 32) {
-      if (nap) __nanosleep(nap);
-      w = ld_relaxed(cell);
-    }
-  }
+  if (fast) w = cell_await(cell, w, ctx.last_ticket);               // tagged cell: wait for the store of THIS tenure of idx
   *out = (uint32_t)w;
   const uint32_t fl = (q.flags & kFencedPayload) ? q.flags : (q.flags | kRelaxedInstall);
   Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, fl, paired, t);

@@ -98,7 +98,8 @@ struct Ymc {
     YmcCell* c = cell(q, i);
     uint64_t w = ld_acquire(&c->val);
     if (w == kBot && park_ns && (q.flags & kEagerEmpty) && ld_relaxed(q.tail) <= i) park_ns = 0;   // no enqueuer holds cell i yet
-    for (uint32_t waited = 0, nap = 32; w == kBot && waited < park_ns; waited += nap, nap = nap * 2 < q.park_nap ? nap * 2 : q.park_nap) {
+    const uint32_t nap_cap = q.park_nap < 32 ? 32u : q.park_nap;
+    for (uint32_t waited = 0, nap = 32; w == kBot && waited < park_ns; waited += nap, nap = nap * 2 < nap_cap ? nap * 2 : nap_cap) {
       __nanosleep(nap);                                       // D2: bounded wait on the own cell
       w = ld_acquire(&c->val);
     }
@@ -145,8 +146,11 @@ struct Ymc {
     if (!(s & kPending) || id_of(s) < id) return;
     s = ld_acquire(&r->deq_state);
     uint64_t prior = id, i = id, cand = 0;
+    [[maybe_unused]] uint32_t sn = 0;
     for (;;) {
+      if (GQ_STUCK(sn, 40, me, &r->deq_state, &r->deq_id, q.head, q.tail)) return;
       while (!cand && id_of(s) == prior) {                    // look for a candidate cell
+        if (GQ_STUCK(sn, 41, me, &r->deq_state, &r->deq_id, q.head, q.tail)) return;
         ++i;
         const uint64_t w = help_enq(q, me, i, 0);
         if (w == kEmptyRet || (w != kTop && ld_acquire32(&cell(q, i)->deq) == kBot32)) cand = i;
@@ -209,7 +213,9 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
   ++h->n_slow_enq;
   st_release(&h->enq_val, val);                               // payload first, then the state word (P:L284 discipline)
   st_release(&h->enq_state, Y::kPending | id);
+  [[maybe_unused]] uint32_t sn = 0;
   do {
+    if (GQ_STUCK(sn, 42, ctx.tid, &h->enq_state, q.head, q.tail)) break;
     const uint64_t i = Y::take<false, kWarpFaa>(q.tail);
     if (i >= Y::last(q)) {                                    // pool ran out: withdraw unless a helper already placed it
       Y::pool_exhausted(q);
@@ -260,7 +266,7 @@ __device__ __forceinline__ int dequeue(const YmcView& q, thread_ctx& ctx, uint32
       break;
     }
     // the claim is decided on this one word against the helpers' CAS (help_deq); the value is already in hand: relaxed
-    if (w != Y::kTop && cas_relaxed32(&Y::cell(q, i)->deq, Y::kBot32, Y::kTop32) == Y::kBot32) { ctx.last_ticket = i; break; }   // value claimed
+    if (w != Y::kTop && (GQ_MUT(MUT_YMC_NO_CLAIM) || cas_relaxed32(&Y::cell(q, i)->deq, Y::kBot32, Y::kTop32) == Y::kBot32)) { ctx.last_ticket = i; break; }   // value claimed
     w = Y::kTop;
     id = i;
     if (retries) ++*retries;

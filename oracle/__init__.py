@@ -59,6 +59,16 @@ def lib():
             L.orc_rt_render.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, _f32p,
                                         C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _f32p, C.POINTER(C.c_uint64)]
             L.orc_rt_render.restype = None
+            L.orc_rt_fmix32.argtypes = [C.c_uint32]
+            L.orc_rt_fmix32.restype = C.c_uint32
+            L.orc_rt_rnd.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32]
+            L.orc_rt_rnd.restype = C.c_float
+            L.orc_rt_camera_ray.argtypes = [C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_float, C.c_float, _f32p]
+            L.orc_rt_camera_ray.restype = None
+            L.orc_rt_nearest_hit.argtypes = [C.c_uint32, _f32p, _f32p, _f32p, C.POINTER(C.c_float)]
+            L.orc_rt_nearest_hit.restype = C.c_int
+            L.orc_rt_scatter.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _f32p, _f32p]
+            L.orc_rt_scatter.restype = None
         _lib = L
     return _lib
 
@@ -211,3 +221,34 @@ def rt_render(width, height, spp, max_bounce, spheres, seed, threads=0, row0=0, 
     lib().orc_rt_render(width, height, spp, max_bounce, sp.shape[0], sp.reshape(-1), int(seed), int(threads),
                         int(row0), int(row1), img.reshape(-1), C.byref(rays))
     return img, rays.value
+
+
+# ---- the tracer's steps one by one (apps_cpu.cpp), so that tests can pin each against something other than itself
+def rt_fmix32(x) -> int:
+    return int(lib().orc_rt_fmix32(int(x) & 0xFFFFFFFF))
+
+
+def rt_rnd(seed, pixel, sample, bounce, dim) -> float:
+    return float(lib().orc_rt_rnd(int(seed), int(pixel), int(sample), int(bounce), int(dim)))
+
+
+def rt_camera_ray(width, height, px, py, u0, u1):
+    """(origin[3], direction[3]) of the primary ray through pixel (px, py) with sub-pixel jitter (u0, u1)."""
+    out = np.zeros(6, np.float32)
+    lib().orc_rt_camera_ray(int(width), int(height), int(px), int(py), float(u0), float(u1), out)
+    return out[:3].copy(), out[3:].copy()
+
+
+def rt_nearest_hit(spheres, origin, direction):
+    """(sphere index or -1, t) of the nearest hit with t > t_min."""
+    sp = np.ascontiguousarray(spheres, np.float32)
+    t = C.c_float(0)
+    i = lib().orc_rt_nearest_hit(sp.shape[0], sp.reshape(-1) if sp.size else np.zeros(8, np.float32),
+                                 np.ascontiguousarray(origin, np.float32), np.ascontiguousarray(direction, np.float32), C.byref(t))
+    return int(i), float(t.value)
+
+
+def rt_scatter(seed, pixel, sample, bounce, normal):
+    out = np.zeros(3, np.float32)
+    lib().orc_rt_scatter(int(seed), int(pixel), int(sample), int(bounce), np.ascontiguousarray(normal, np.float32), out)
+    return out

@@ -11,11 +11,20 @@
 //                 disconnected graphs; |d[u]-d[v]| <= 1 across every edge; parent at d-1.
 //
 //  orc_rt_render  the path tracer of BASELINE.json config 5 with the paper-silent constants of
-//                 DESIGN.md §6, one pixel at a time.  fp32, every operation individually rounded
-//                 (built with -ffp-contract=off, no fast-math).
-//                 Pins: empty scene = background; one sphere on the axis: analytic primary hit;
-//                 emissive sphere: 4 x albedo where hit.  The full 256-sphere image has no
-//                 independent pin: parity unpinned beyond those closed forms.
+//                 DESIGN.md §6, one (pixel, sample) path at a time, written as the textbook loop
+//                 "camera ray; repeat { nearest hit; shade; scatter }" over explicit Ray / Hit records.
+//                 fp32, every operation individually rounded (built with -ffp-contract=off, no fast-math).
+//                 Each step is exported on its own (orc_rt_fmix32, orc_rt_rnd, orc_rt_camera_ray,
+//                 orc_rt_nearest_hit, orc_rt_scatter) so that tests/test_oracle_apps.py can pin it
+//                 against something other than itself:
+//                   fmix32      published MurmurHash3 finaliser values; its published inverse undoes it
+//                   rnd         range, 2^-24 grid, uniformity and independence across dims (chi-square)
+//                   camera ray  pinhole geometry in float64
+//                   nearest hit float64 quadratic formula over all spheres; t_min; ties -> lowest index
+//                   scatter     unit length, hemisphere of the normal, E[cos] = 2/3 (cosine law)
+//                   image       closed forms: background, emissive silhouette, grey sphere in an emissive
+//                               shell (one bounce), coincident spheres, occlusion, closed diffuse room
+//                               (absorption at the depth limit, ray count), sky view factor (1+cos)/2
 #include <cmath>
 #include <cstdint>
 #include <thread>
@@ -46,91 +55,125 @@ void orc_bfs(uint32_t nv, const uint64_t* rowptr, const uint32_t* col, uint32_t 
 // ------------------------------------------------------------------------------------- tracer
 namespace {
 
-struct V3 { float x, y, z; };
-inline V3 add(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
-inline V3 sub(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
-inline V3 mul(V3 a, V3 b) { return {a.x * b.x, a.y * b.y, a.z * b.z}; }
-inline V3 scale(V3 a, float s) { return {a.x * s, a.y * s, a.z * s}; }
-inline V3 divs(V3 a, float s) { return {a.x / s, a.y / s, a.z / s}; }
-inline float dot(V3 a, V3 b) { return (a.x * b.x + a.y * b.y) + a.z * b.z; }
-
-// murmur3 32-bit finaliser, applied three times over (seed, pixel, sample, bounce, dim)
-inline uint32_t fmix32(uint32_t x) {
-  x ^= x >> 16; x *= 0x85ebca6bu; x ^= x >> 13; x *= 0xc2b2ae35u; x ^= x >> 16;
-  return x;
-}
-inline float rnd(uint64_t seed, uint32_t pixel, uint32_t sample, uint32_t bounce, uint32_t dim) {
-  uint32_t x = fmix32((uint32_t)seed ^ (pixel * 0x9E3779B1u));
-  x = fmix32(x ^ (sample * 0x85EBCA77u + bounce * 0xC2B2AE3Du + dim * 0x27D4EB2Fu));
-  x = fmix32(x ^ (uint32_t)(seed >> 32));
-  return (float)(x >> 8) * (1.0f / 16777216.0f);
-}
-
+struct Vec { float x, y, z; };
+struct Ray { Vec origin, dir; };
+struct Hit { int sphere; float t; };                       // sphere < 0: miss
+struct Sphere { Vec centre; float radius; Vec albedo; bool emissive; };
 struct Scene { uint32_t w, h, spp, max_bounce, ns; const float* sp; uint64_t seed; };
 
-constexpr float kTMin = 1e-3f;
-constexpr float kHalfH = 0.36397023f;           // tan(20 deg): vertical FOV 40 deg
-const V3 kEye = {0.0f, 0.0f, 35.0f};
-const V3 kBackground = {0.7f, 0.8f, 1.0f};
+inline Vec operator+(Vec a, Vec b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline Vec operator-(Vec a, Vec b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline Vec operator*(Vec a, Vec b) { return {a.x * b.x, a.y * b.y, a.z * b.z}; }
+inline Vec operator*(Vec a, float s) { return {a.x * s, a.y * s, a.z * s}; }
+inline Vec operator/(Vec a, float s) { return {a.x / s, a.y / s, a.z / s}; }
+inline float dot(Vec a, Vec b) { return (a.x * b.x + a.y * b.y) + a.z * b.z; }      // (x + y) + z
+inline Vec unit(Vec a) { return a / std::sqrt(dot(a, a)); }
 
-// radiance of one (pixel, sample) path; *rays += ray segments traced
-V3 trace_path(const Scene& sc, uint32_t px, uint32_t py, uint32_t s, uint64_t* rays) {
-  const uint32_t pixel = py * sc.w + px;
+inline Sphere sphere_at(const Scene& sc, uint32_t i) {
+  const float* S = sc.sp + 8 * i;
+  return Sphere{{S[0], S[1], S[2]}, S[3], {S[4], S[5], S[6]}, S[7] != 0.0f};
+}
+
+// DESIGN.md §6 RNG: three rounds of the 32-bit MurmurHash3 finaliser over (seed, pixel, sample, bounce, dim)
+uint32_t fmix32(uint32_t h) {
+  h ^= h >> 16;
+  h *= 0x85ebca6bu;
+  h ^= h >> 13;
+  h *= 0xc2b2ae35u;
+  h ^= h >> 16;
+  return h;
+}
+float rnd(uint64_t seed, uint32_t pixel, uint32_t sample, uint32_t bounce, uint32_t dim) {
+  const uint32_t seed_lo = (uint32_t)seed, seed_hi = (uint32_t)(seed >> 32);
+  const uint32_t key = sample * 0x85EBCA77u + bounce * 0xC2B2AE3Du + dim * 0x27D4EB2Fu;
+  uint32_t h = fmix32(seed_lo ^ (pixel * 0x9E3779B1u));
+  h = fmix32(h ^ key);
+  h = fmix32(h ^ seed_hi);
+  return (float)(h >> 8) * (1.0f / 16777216.0f);          // 24 high bits: a multiple of 2^-24 in [0, 1)
+}
+
+constexpr float kTMin = 1e-3f;
+constexpr float kTanHalfFov = 0.36397023f;                 // tan(20 deg): vertical field of view 40 deg
+const Vec kEye = {0.0f, 0.0f, 35.0f};
+const Vec kBackground = {0.7f, 0.8f, 1.0f};
+constexpr float kEmission = 4.0f;
+
+// pinhole camera at kEye looking down -z, up +y; (u0, u1) = sub-pixel jitter
+Ray camera_ray(const Scene& sc, uint32_t px, uint32_t py, float u0, float u1) {
   const float aspect = (float)sc.w / (float)sc.h;
-  const float u0 = rnd(sc.seed, pixel, s, 0, 0), u1 = rnd(sc.seed, pixel, s, 0, 1);
   const float sx = (((float)px + u0) / (float)sc.w) * 2.0f - 1.0f;
   const float sy = 1.0f - (((float)py + u1) / (float)sc.h) * 2.0f;
-  V3 d = {sx * (kHalfH * aspect), sy * kHalfH, -1.0f};
-  d = divs(d, std::sqrt(dot(d, d)));
-  V3 o = kEye, T = {1.0f, 1.0f, 1.0f}, L = {0.0f, 0.0f, 0.0f};
-  for (uint32_t b = 0; b <= sc.max_bounce; ++b) {
-    ++*rays;
-    float best_t = INFINITY;
-    int best = -1;
-    for (uint32_t i = 0; i < sc.ns; ++i) {             // brute force, ties -> lowest index
-      const float* S = sc.sp + 8 * i;
-      const V3 oc = sub(o, V3{S[0], S[1], S[2]});
-      const float bq = dot(oc, d);
-      const float cq = dot(oc, oc) - S[3] * S[3];
-      const float disc = bq * bq - cq;
-      if (disc < 0.0f) continue;
-      const float sq = std::sqrt(disc);
-      float t = -bq - sq;
-      if (!(t > kTMin)) { t = -bq + sq; if (!(t > kTMin)) continue; }
-      if (t < best_t) { best_t = t; best = (int)i; }
-    }
-    if (best < 0) { L = add(L, mul(T, kBackground)); break; }
-    const float* S = sc.sp + 8 * best;
-    const V3 albedo = {S[4], S[5], S[6]};
-    if (S[7] != 0.0f) { L = add(L, mul(T, scale(albedo, 4.0f))); break; }   // emissive: 4 x albedo, path ends
-    T = mul(T, albedo);
-    if (b == sc.max_bounce) break;                                          // absorbed
-    const V3 p = add(o, scale(d, best_t));
-    const V3 n = divs(sub(p, V3{S[0], S[1], S[2]}), S[3]);
-    V3 unit = n;                                                            // fallback after 16 rejections
-    for (uint32_t k = 0; k < 16; ++k) {
-      const V3 v = {2.0f * rnd(sc.seed, pixel, s, b, 2 + 3 * k) - 1.0f,
-                    2.0f * rnd(sc.seed, pixel, s, b, 3 + 3 * k) - 1.0f,
-                    2.0f * rnd(sc.seed, pixel, s, b, 4 + 3 * k) - 1.0f};
-      const float l2 = dot(v, v);
-      if (l2 <= 1.0f && l2 > 1e-12f) { unit = divs(v, std::sqrt(l2)); break; }
-    }
-    V3 sdir = add(n, unit);
-    float l2 = dot(sdir, sdir);
-    if (!(l2 > 1e-12f)) { sdir = n; l2 = dot(n, n); }
-    d = divs(sdir, std::sqrt(l2));
-    o = p;
+  return Ray{kEye, unit(Vec{sx * (kTanHalfFov * aspect), sy * kTanHalfFov, -1.0f})};
+}
+
+// smallest t > kTMin over all spheres (|d| = 1: t = -b -+ sqrt(b^2 - c)); equal t: the lowest index wins
+Hit nearest_hit(const Scene& sc, const Ray& ray) {
+  Hit best{-1, INFINITY};
+  for (uint32_t i = 0; i < sc.ns; ++i) {
+    const Sphere s = sphere_at(sc, i);
+    const Vec oc = ray.origin - s.centre;
+    const float b = dot(oc, ray.dir);
+    const float c = dot(oc, oc) - s.radius * s.radius;
+    const float disc = b * b - c;
+    if (disc < 0.0f) continue;
+    const float root = std::sqrt(disc);
+    float t = -b - root;                                   // near root first, else the far one (origin inside)
+    if (!(t > kTMin)) t = -b + root;
+    if (!(t > kTMin)) continue;
+    if (t < best.t) best = Hit{(int)i, t};
   }
-  return L;
+  return best;
+}
+
+// Lambertian direction: normalize(n + u), u a unit vector by rejection sampling in the unit ball
+// (try k uses dims 2+3k .. 4+3k; at most 16 tries, then u = n)
+Vec scatter(const Scene& sc, uint32_t pixel, uint32_t sample, uint32_t bounce, Vec n) {
+  Vec u = n;
+  for (uint32_t k = 0; k < 16; ++k) {
+    const Vec v = {2.0f * rnd(sc.seed, pixel, sample, bounce, 2 + 3 * k) - 1.0f,
+                   2.0f * rnd(sc.seed, pixel, sample, bounce, 3 + 3 * k) - 1.0f,
+                   2.0f * rnd(sc.seed, pixel, sample, bounce, 4 + 3 * k) - 1.0f};
+    const float len2 = dot(v, v);
+    if (len2 <= 1.0f && len2 > 1e-12f) { u = v / std::sqrt(len2); break; }
+  }
+  Vec s = n + u;
+  float len2 = dot(s, s);
+  if (!(len2 > 1e-12f)) { s = n; len2 = dot(n, n); }
+  return s / std::sqrt(len2);
+}
+
+// One bounce of one path.  Returns true while the path lives; when it ends *radiance is its value.
+bool bounce_once(const Scene& sc, uint32_t pixel, uint32_t sample, uint32_t depth, Ray* ray, Vec* throughput, Vec* radiance) {
+  const Hit hit = nearest_hit(sc, *ray);
+  if (hit.sphere < 0) { *radiance = *throughput * kBackground; return false; }
+  const Sphere s = sphere_at(sc, (uint32_t)hit.sphere);
+  if (s.emissive) { *radiance = *throughput * (s.albedo * kEmission); return false; }
+  *throughput = *throughput * s.albedo;
+  if (depth == sc.max_bounce) { *radiance = Vec{0.0f, 0.0f, 0.0f}; return false; }      // absorbed at the depth limit
+  const Vec p = ray->origin + ray->dir * hit.t;
+  const Vec n = (p - s.centre) / s.radius;
+  *ray = Ray{p, scatter(sc, pixel, sample, depth, n)};
+  return true;
+}
+
+// radiance of one (pixel, sample) path; *rays += ray segments traced
+Vec trace_path(const Scene& sc, uint32_t px, uint32_t py, uint32_t sample, uint64_t* rays) {
+  const uint32_t pixel = py * sc.w + px;
+  Ray ray = camera_ray(sc, px, py, rnd(sc.seed, pixel, sample, 0, 0), rnd(sc.seed, pixel, sample, 0, 1));
+  Vec throughput = {1.0f, 1.0f, 1.0f}, radiance = {0.0f, 0.0f, 0.0f};
+  for (uint32_t depth = 0;; ++depth) {
+    ++*rays;
+    if (!bounce_once(sc, pixel, sample, depth, &ray, &throughput, &radiance)) return radiance;
+  }
 }
 
 void render_rows(const Scene& sc, uint32_t y0, uint32_t y1, float* rgb, uint64_t* rays) {
   uint64_t r = 0;
   for (uint32_t py = y0; py < y1; ++py)
     for (uint32_t px = 0; px < sc.w; ++px) {
-      V3 acc = {0.0f, 0.0f, 0.0f};
-      for (uint32_t s = 0; s < sc.spp; ++s) acc = add(acc, trace_path(sc, px, py, s, &r));   // fixed order
-      const V3 c = divs(acc, (float)sc.spp);
+      Vec acc = {0.0f, 0.0f, 0.0f};
+      for (uint32_t s = 0; s < sc.spp; ++s) acc = acc + trace_path(sc, px, py, s, &r);   // samples in order
+      const Vec c = acc / (float)sc.spp;
       float* out = rgb + 3 * ((size_t)py * sc.w + px);
       out[0] = c.x; out[1] = c.y; out[2] = c.z;
     }
@@ -139,8 +182,31 @@ void render_rows(const Scene& sc, uint32_t y0, uint32_t y1, float* rgb, uint64_t
 
 }  // namespace
 
-extern "C" void orc_rt_render(uint32_t w, uint32_t h, uint32_t spp, uint32_t max_bounce, uint32_t ns, const float* spheres,
-                              uint64_t seed, uint32_t threads, uint32_t row0, uint32_t row1, float* rgb, uint64_t* rays_out) {
+extern "C" {
+
+uint32_t orc_rt_fmix32(uint32_t x) { return fmix32(x); }
+float orc_rt_rnd(uint64_t seed, uint32_t pixel, uint32_t sample, uint32_t bounce, uint32_t dim) { return rnd(seed, pixel, sample, bounce, dim); }
+// out6 = origin xyz, direction xyz
+void orc_rt_camera_ray(uint32_t w, uint32_t h, uint32_t px, uint32_t py, float u0, float u1, float* out6) {
+  Scene sc{w, h, 1, 0, 0, nullptr, 0};
+  const Ray r = camera_ray(sc, px, py, u0, u1);
+  out6[0] = r.origin.x; out6[1] = r.origin.y; out6[2] = r.origin.z; out6[3] = r.dir.x; out6[4] = r.dir.y; out6[5] = r.dir.z;
+}
+// returns the sphere index (-1 = miss), *t_out = hit distance
+int orc_rt_nearest_hit(uint32_t ns, const float* spheres, const float* origin3, const float* dir3, float* t_out) {
+  Scene sc{1, 1, 1, 0, ns, spheres, 0};
+  const Hit h = nearest_hit(sc, Ray{{origin3[0], origin3[1], origin3[2]}, {dir3[0], dir3[1], dir3[2]}});
+  *t_out = h.t;
+  return h.sphere;
+}
+void orc_rt_scatter(uint64_t seed, uint32_t pixel, uint32_t sample, uint32_t bounce, const float* normal3, float* out3) {
+  Scene sc{1, 1, 1, 0, 0, nullptr, seed};
+  const Vec d = scatter(sc, pixel, sample, bounce, Vec{normal3[0], normal3[1], normal3[2]});
+  out3[0] = d.x; out3[1] = d.y; out3[2] = d.z;
+}
+
+void orc_rt_render(uint32_t w, uint32_t h, uint32_t spp, uint32_t max_bounce, uint32_t ns, const float* spheres,
+                   uint64_t seed, uint32_t threads, uint32_t row0, uint32_t row1, float* rgb, uint64_t* rays_out) {
   Scene sc{w, h, spp, max_bounce, ns, spheres, seed};
   if (row1 > h) row1 = h;
   if (row0 >= row1) { *rays_out = 0; return; }
@@ -158,3 +224,5 @@ extern "C" void orc_rt_render(uint32_t w, uint32_t h, uint32_t spp, uint32_t max
   for (uint64_t r : rays) total += r;
   *rays_out = total;
 }
+
+}  // extern "C"

@@ -10,6 +10,8 @@ import os
 
 import numpy as np
 
+import contextlib
+
 from .build import LIB, build as _build
 
 GQ_LFQ, GQ_WFQ, GQ_WFQ_YMC, GQ_LFQ_DIRECT = 0, 1, 2, 3
@@ -19,6 +21,8 @@ GQ_E_INVAL, GQ_E_NOMEM, GQ_E_CUDA, GQ_E_RESIDENCY, GQ_E_TIMEOUT, GQ_E_STATE, GQ_
 GQ_PATIENCE_ZERO = 0xFFFFFFFF
 GQ_F_PER_LANE_FAA, GQ_F_NO_PROBE, GQ_F_NO_DEQ_SPIN, GQ_F_NO_OPT_CAS, GQ_F_PLAIN_THR_STORE = 1, 2, 4, 8, 16
 GQ_F_THR_FIRST, GQ_F_NO_PAIRED_FAA, GQ_F_THR_RED_MAX, GQ_F_FENCED_PAYLOAD, GQ_F_EAGER_EMPTY, GQ_F_NO_CELL_PREFETCH, GQ_F_NO_FULL_TEST = 32, 64, 128, 256, 512, 1024, 2048
+GQ_F_NO_REPAIR = 4096
+GQ_PARK_SPIN_NONE = 0xFFFFFFFF
 KIND_NAMES = {GQ_LFQ: "G-LFQ", GQ_WFQ: "G-WFQ", GQ_WFQ_YMC: "G-WFQ-YMC", GQ_LFQ_DIRECT: "G-LFQ-D"}
 _ERR = {-1: "INVAL", -2: "NOMEM", -3: "CUDA", -4: "RESIDENCY", -5: "TIMEOUT", -6: "STATE", -7: "POOL"}
 
@@ -34,7 +38,7 @@ class gq_opts(C.Structure):
     _fields_ = [("max_threads", C.c_uint32), ("enq_patience", C.c_uint32), ("deq_patience", C.c_uint32),
                 ("help_delay", C.c_uint32), ("ymc_pool_cells", C.c_uint64), ("storage", C.c_void_p),
                 ("storage_bytes", C.c_size_t), ("layout", C.c_uint32), ("flags", C.c_uint32),
-                ("park_ns", C.c_uint32), ("park_nap_ns", C.c_uint32)]
+                ("park_ns", C.c_uint32), ("park_nap_ns", C.c_uint32), ("park_spin_ns", C.c_uint32), ("reserved", C.c_uint32)]
 
 
 class gq_run_cfg(C.Structure):
@@ -42,7 +46,7 @@ class gq_run_cfg(C.Structure):
                 ("duration_ms", C.c_double), ("producer_fraction", C.c_double), ("seed", C.c_uint64),
                 ("record_history", C.c_uint32), ("ops_per_thread", C.c_uint32), ("jitter_ns", C.c_uint32),
                 ("fail_backoff_ns", C.c_uint32), ("value_base", C.c_uint64),
-                ("role_layout", C.c_uint32), ("reserved", C.c_uint32)]
+                ("role_layout", C.c_uint32), ("converged", C.c_uint32)]
 
 
 class gq_run_result(C.Structure):
@@ -83,11 +87,12 @@ HIST_DTYPE = np.dtype([("proc", "<u4"), ("op", "<u4"), ("arg", "<u4"), ("ret_sta
 SYMBOLS = ("queue_storage_bytes", "queue_create", "queue_create_ex", "queue_destroy", "queue_reset", "queue_prefill",
            "queue_drain", "queue_device_view", "queue_kind", "queue_max_coresident_threads", "run_balanced",
            "run_split", "run_faa_ceiling", "run_slot_atomic_ceiling", "run_warp_faa_probe", "queue_run_script",
-           "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "gq_last_cuda_error", "gq_version")
+           "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "gq_last_cuda_error", "gq_version",
+           "gq_dbg_sites", "gq_dbg_trace", "gq_set_mutation", "queue_debug_counters")
 
 
-def _load():
-    path = _build()          # compiles with nvcc when sources are newer than the .so
+def _load(variant=""):
+    path = _build(variant=variant)          # compiles with nvcc when sources are newer than the .so
     L = C.CDLL(path)
     P = C.POINTER
     L.queue_storage_bytes.argtypes = [C.c_int, C.c_uint64, P(gq_opts)]
@@ -100,6 +105,7 @@ def _load():
     L.queue_drain.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(C.c_uint64), C.c_void_p]
     L.queue_device_view.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
     L.queue_kind.argtypes = [C.c_void_p]
+    L.queue_debug_counters.argtypes = [C.c_void_p, C.c_void_p]
     L.queue_max_coresident_threads.argtypes = [C.c_int, C.c_int, P(C.c_uint32)]
     L.run_balanced.argtypes = [C.c_void_p, P(gq_run_cfg), P(gq_run_result)]
     L.run_split.argtypes = [C.c_void_p, P(gq_run_cfg), P(gq_run_result)]
@@ -113,10 +119,25 @@ def _load():
     L.rt_render.argtypes = [C.c_int, P(gq_rt_scene), C.c_void_p, P(gq_rt_stats), C.c_void_p]
     L.gq_last_cuda_error.restype = C.c_char_p
     L.gq_version.restype = C.c_char_p
+    L.gq_dbg_sites.argtypes = [C.c_void_p]
+    L.gq_dbg_trace.argtypes = [C.c_void_p, C.c_uint64, P(C.c_uint64)]
+    L.gq_set_mutation.argtypes = [C.c_uint32]
     return L
 
 
 lib = _load()
+
+
+@contextlib.contextmanager
+def use_variant(variant):
+    """Route every call of this module to another build of the same library (build.py VARIANTS: "mutants", "dbg")
+    for the duration of the block.  Handles must not cross the boundary."""
+    global lib
+    saved, lib = lib, _load(variant)
+    try:
+        yield lib
+    finally:
+        lib = saved
 
 
 def _chk(rc, where):
@@ -163,6 +184,23 @@ def queue_drain(q, max_items, stream=None):
     n = C.c_uint64(0)
     _chk(lib.queue_drain(q, _np_ptr(out), int(max_items), C.byref(n), stream), "queue_drain")
     return out[: n.value].copy()
+
+
+def queue_debug_counters(q):
+    """dict of the hot words of a quiescent queue (gq.h)."""
+    out = np.zeros(16, np.uint64)
+    _chk(lib.queue_debug_counters(q, _np_ptr(out)), "queue_debug_counters")
+    k = lib.queue_kind(q)
+    if k == GQ_WFQ_YMC:
+        return {"head": int(out[0]), "tail": int(out[1]), "N": int(out[6]), "max_threads": int(out[7])}
+    d = {"aq_head": int(out[0]), "aq_tail": int(out[1]), "aq_threshold": int(out[2].astype(np.int64)), "N": int(out[6]), "max_threads": int(out[7])}
+    if k != GQ_LFQ_DIRECT:
+        d.update(fq_head=int(out[3]), fq_tail=int(out[4]), fq_threshold=int(out[5].astype(np.int64)))
+    if k == GQ_WFQ:
+        names = ("tail_inc", "tail_clr", "head_inc", "head_clr")
+        d.update({f"aq_{n}": int(out[8 + i]) for i, n in enumerate(names)})
+        d.update({f"fq_{n}": int(out[12 + i]) for i, n in enumerate(names)})
+    return d
 
 
 def queue_max_coresident_threads(kind, block_threads=256):
@@ -230,6 +268,27 @@ def history_dump(q, max_records=1 << 24):
     n = C.c_uint64(0)
     _chk(lib.history_dump(q, _np_ptr(out), max_records, C.byref(n)), "history_dump")
     return out[: n.value].copy()
+
+
+TRACE_DTYPE = np.dtype([("ns", "<u8"), ("site_tid", "<u8"), ("ticket", "<u8"), ("entry", "<u8"), ("head", "<u8"),
+                        ("tail", "<u8"), ("thr", "<i8"), ("aux", "<u8")])
+
+
+def gq_dbg_sites():
+    out = np.zeros(80, np.uint64)
+    _chk(lib.gq_dbg_sites(_np_ptr(out)), "gq_dbg_sites")
+    return out
+
+
+def gq_dbg_trace(max_records=1 << 16):
+    out = np.empty(max_records, TRACE_DTYPE)
+    n = C.c_uint64(0)
+    _chk(lib.gq_dbg_trace(_np_ptr(out), max_records, C.byref(n)), "gq_dbg_trace")
+    return out[: n.value].copy()
+
+
+def gq_set_mutation(mutation_id):
+    _chk(lib.gq_set_mutation(mutation_id), "gq_set_mutation")
 
 
 def bfs_run(kind, d_rowptr, d_col, nv, src, d_dist, stream=None):

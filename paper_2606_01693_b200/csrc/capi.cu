@@ -31,7 +31,7 @@ static int cuda_fail(cudaError_t e, const char* what) { return gq_cuda_fail(e, w
 extern "C" const char* gq_last_cuda_error(void) { return g_err; }
 extern "C" const char* gq_version(void) { return "gq 0.1 (sm_100a)"; }
 
-static_assert(sizeof(gq_opts) == 56 && sizeof(gq_run_cfg) == 72 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
+static_assert(sizeof(gq_opts) == 64 && sizeof(gq_run_cfg) == 72 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
               "ABI structs: the Python binding mirrors these layouts");
 
 // ------------------------------------------------------------------------------- handle
@@ -86,7 +86,7 @@ struct Layout {
   size_t off_hot = 0, off_aq = 0, off_fq = 0, off_data = 0, off_owner_aq = 0, off_owner_fq = 0, off_rec = 0, off_rec_fq = 0, off_pool = 0;
   size_t total = 0;
   uint64_t pool_cells = 0;
-  uint32_t park_ns = 0, park_nap = 0, prefetch_dist = 0;
+  uint32_t park_ns = 0, park_nap = 0, prefetch_dist = 0, spin_ns = 0;
 };
 
 template <class Q> static int max_blocks_per_sm(int block_threads);
@@ -101,7 +101,8 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
   if (k == 0) k = 148 * 2048;                         // no device visible: size for a full B200
   *max_threads_out = k;
   L->park_ns = o->park_ns ? o->park_ns : 250000u;
-  L->park_nap = o->park_nap_ns ? std::max(o->park_nap_ns, 32u) : 128u;
+  L->park_nap = o->park_nap_ns ? (o->park_nap_ns < 32u ? 0u : o->park_nap_ns) : 128u;
+  L->spin_ns = o->park_spin_ns == GQ_PARK_SPIN_NONE ? 0u : (o->park_spin_ns ? o->park_spin_ns : 2000u);
   L->prefetch_dist = (o->flags & GQ_F_NO_CELL_PREFETCH) ? 0u : k;
   size_t off = 0;
   L->off_hot = off; off += 16 * kHotStride;
@@ -182,6 +183,8 @@ static RingView make_ring(char* base, const Layout& L, size_t off_entries, size_
   // rings of 32 MiB and more (BFS frontier queues) do not stay in L2 next to the graph: prefetch k tickets ahead
   const size_t ring_bytes = (size_t)(2 * L.N) * (8u << L.slot_shift);
   r.prefetch = ring_bytes >= (32u << 20) ? L.prefetch_dist : 0;
+  r.id = hot_slot ? 1u : 0u;
+  r.spin_ns = L.spin_ns;
   return r;
 }
 
@@ -297,6 +300,7 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
   if (!q) return GQ_E_NOMEM;
   q->kind = kind; q->capacity = capacity; q->N = L.N; q->max_threads = k;
   if (opts) q->opts = *opts;
+  q->opts.flags &= kPublicFlags;        // internal flag bits (ring.cuh) cannot be set from outside
   q->bytes = L.total;
   if (opts && opts->storage) {
     if (opts->storage_bytes < L.total || (reinterpret_cast<uintptr_t>(opts->storage) & 255)) { delete q; return GQ_E_INVAL; }
@@ -375,6 +379,42 @@ extern "C" int queue_reset(gq_queue* q, void* stream) {
 }
 
 extern "C" int queue_kind(const gq_queue* q) { return q ? q->kind : GQ_E_INVAL; }
+
+__global__ void wfq_rounds_kernel(const WfqRecord* a, uint32_t n, uint64_t* out4) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  uint64_t v[4] = {0, 0, 0, 0};
+  if (i < n) { v[0] = a[i].n_tail_inc; v[1] = a[i].n_tail_clr; v[2] = a[i].n_head_inc; v[3] = a[i].n_head_clr; }
+  for (int k = 0; k < 4; ++k) { const uint64_t s = warp_sum(v[k]); if ((threadIdx.x & 31) == 0 && s) red_add_relaxed(out4 + k, s); }
+}
+// Quiescent read-back of the hot words (Lemma III.7 tests, diagnostics): ticket counters decoded from their packed form.
+extern "C" int queue_debug_counters(gq_queue* q, uint64_t* out8 /* 16 words */) {
+  if (!q || !out8) return GQ_E_INVAL;
+  CU(cudaDeviceSynchronize());
+  std::memset(out8, 0, 16 * sizeof(uint64_t));
+  auto rd = [](const void* p, uint64_t* v) { return cudaMemcpy(v, p, 8, cudaMemcpyDeviceToHost); };
+  auto ring = [&](const RingView& r, int shift, uint64_t* o) -> cudaError_t {
+    cudaError_t e = rd(r.head, o); if (e == cudaSuccess) e = rd(r.tail, o + 1); if (e == cudaSuccess) e = rd(r.threshold, o + 2);
+    o[0] >>= shift; o[1] >>= shift;
+    return e;
+  };
+  cudaError_t e = cudaSuccess;
+  if (q->kind == GQ_LFQ) { e = ring(q->lfq.aq, 0, out8); if (e == cudaSuccess) e = ring(q->lfq.fq, 0, out8 + 3); }
+  else if (q->kind == GQ_WFQ) { e = ring(q->wfq.aq, WfqFmt::kCtrShift, out8); if (e == cudaSuccess) e = ring(q->wfq.fq, WfqFmt::kCtrShift, out8 + 3); }
+  else if (q->kind == GQ_LFQ_DIRECT) e = ring(q->dlfq.r, 0, out8);
+  else { e = rd(q->ymc.head, out8); if (e == cudaSuccess) e = rd(q->ymc.tail, out8 + 1); }
+  out8[6] = q->N; out8[7] = q->max_threads;
+  if (e == cudaSuccess && q->kind == GQ_WFQ) {          // slow-path rounds since the last reset (Lemma III.7)
+    uint64_t* d = nullptr;
+    CU(cudaMalloc(&d, 64));
+    cudaMemset(d, 0, 64);
+    const unsigned g = (q->max_threads + 255) / 256;
+    wfq_rounds_kernel<<<g, 256>>>(static_cast<const WfqRecord*>(q->wfq.aq.rec), q->max_threads, d);
+    wfq_rounds_kernel<<<g, 256>>>(static_cast<const WfqRecord*>(q->wfq.fq.rec), q->max_threads, d + 4);
+    e = cudaMemcpy(out8 + 8, d, 64, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+  }
+  return e == cudaSuccess ? 0 : cuda_fail(e, "queue_debug_counters");
+}
 
 extern "C" int queue_device_view(const gq_queue* q, void* view_out, size_t view_bytes) {
   if (!q || !view_out) return GQ_E_INVAL;
@@ -496,6 +536,9 @@ static BenchParams make_params(const gq_run_cfg* cfg, const Resolved& r, int mod
   p.prod_threshold = (uint64_t)(pf * 4294967296.0);
   p.seed = (uint32_t)cfg->seed; p.ops_per_thread = cfg->ops_per_thread;
   p.jitter_ns = cfg->jitter_ns; p.fail_backoff_ns = cfg->fail_backoff_ns; p.value_base = cfg->value_base;
+  p.converged = cfg->converged;
+  // history runs small enough for it use the payload encoding of BASELINE.json configs[0]: thread << 16 | iteration
+  p.tid_shift = (cfg->record_history && r.threads <= 65536 && cfg->ops_per_thread <= 65536) ? 16u : 0u;
   return p;
 }
 
@@ -514,15 +557,39 @@ static int finish_run(uint64_t* d_ctr, cudaEvent_t e0, cudaEvent_t e1, const gq_
   return 0;
 }
 
-// debug builds (-DGQ_DEBUG_STUCK=cap): report what the livelock detector recorded
-extern "C" int gq_dbg_sites(unsigned long long* out16) {
+// ---- debug / fault-injection builds (include/gq/detail/debug.cuh); in the product build these return GQ_E_INVAL
+extern "C" int gq_dbg_sites(unsigned long long* out80) {
 #ifdef GQ_DBG_SITES
-  if (cudaMemcpyFromSymbol(out16, gq::detail::g_dbg, 32 * 8) != cudaSuccess) return -1;
-  unsigned long long z[32] = {0};
-  cudaMemcpyToSymbol(gq::detail::g_dbg, z, sizeof z);
+  if (!out80) return GQ_E_INVAL;
+  CU(cudaMemcpyFromSymbol(out80, gq::detail::g_dbg, 80 * 8));
+  unsigned long long z[80] = {0};
+  CU(cudaMemcpyToSymbol(gq::detail::g_dbg, z, sizeof z));
   return 0;
 #else
-  (void)out16; return -1;
+  (void)out80; return GQ_E_INVAL;
+#endif
+}
+extern "C" int gq_dbg_trace(void* out, uint64_t max_records, uint64_t* n_out) {
+#ifdef GQ_DBG_SITES
+  if (!out || !n_out) return GQ_E_INVAL;
+  unsigned long long n = 0, zero = 0;
+  CU(cudaMemcpyFromSymbol(&n, gq::detail::g_trace_n, 8));
+  n = std::min<unsigned long long>(std::min<unsigned long long>(n, gq::detail::kTraceCap), max_records);
+  if (n) CU(cudaMemcpyFromSymbol(out, gq::detail::g_trace, n * sizeof(gq::detail::TraceRec)));
+  CU(cudaMemcpyToSymbol(gq::detail::g_trace_n, &zero, 8));
+  *n_out = n;
+  return 0;
+#else
+  (void)out; (void)max_records; (void)n_out; return GQ_E_INVAL;
+#endif
+}
+extern "C" int gq_set_mutation(uint32_t id) {
+#ifdef GQ_MUTANTS
+  if (id >= gq::detail::MUT_COUNT) return GQ_E_INVAL;
+  CU(cudaMemcpyToSymbol(gq::detail::g_mutation, &id, 4));
+  return 0;
+#else
+  (void)id; return GQ_E_INVAL;
 #endif
 }
 static void report_stuck() {
@@ -548,9 +615,11 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   if (!hist && cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
   const bool fused = mode == MODE_SPLIT && cfg->role_layout == 2;       // mixed warps, one converged call (G-LFQ)
   if (fused && (q->kind != GQ_LFQ || per_lane)) return GQ_E_INVAL;
-  void* fn = fused ? (hist ? (void*)bench_kernel<Q, true, true, true> : (void*)bench_kernel<Q, false, true, true>)
-           : hist ? (per_lane ? (void*)bench_kernel<Q, true, false> : (void*)bench_kernel<Q, true, true>)
-                  : (per_lane ? (void*)bench_kernel<Q, false, false> : (void*)bench_kernel<Q, false, true>);
+  if (hist && per_lane) return GQ_E_INVAL;                              // the per-thread-FAA ablation is a timing variant only
+  void* fn = hist ? (void*)bench_kernel<Q, true, true> : (per_lane ? (void*)bench_kernel<Q, false, false> : (void*)bench_kernel<Q, false, true>);
+  if constexpr (HasFused<Q>::value) {
+    if (fused) fn = hist ? (void*)bench_kernel<Q, true, true, true> : (void*)bench_kernel<Q, false, true, true>;
+  }
   Resolved r;
   int nb = 0;
   const uint32_t blk = cfg->block_threads ? cfg->block_threads : 256;
@@ -688,14 +757,14 @@ extern "C" int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t se
 
 // ------------------------------------------------------------------------------- prefill / drain / script / history
 template <class Q>
-static int prefill_t(const Q& view, const uint32_t* host_vals, uint64_t count, cudaStream_t st, uint32_t serial) {
+static int prefill_t(const Q& view, const uint32_t* host_vals, uint64_t count, cudaStream_t st, uint32_t serial, uint32_t lanes) {
   uint32_t* d_vals = nullptr; uint64_t* d_n = nullptr;
   CU(cudaMalloc(&d_vals, std::max<uint64_t>(count, 1) * 4));
   cudaError_t e = cudaMalloc(&d_n, 8);
   if (e != cudaSuccess) { cudaFree(d_vals); return cuda_fail(e, "cudaMalloc"); }
   uint64_t n_ok = 0;
   e = cudaMemcpyAsync(d_vals, host_vals, count * 4, cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess) { prefill_kernel<Q><<<1, 32, 0, st>>>(view, d_vals, count, d_n, serial); e = cudaGetLastError(); }
+  if (e == cudaSuccess) { prefill_kernel<Q><<<1, 32, 0, st>>>(view, d_vals, count, d_n, serial, lanes); e = cudaGetLastError(); }
   if (e == cudaSuccess) e = cudaMemcpyAsync(&n_ok, d_n, 8, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d_vals); cudaFree(d_n);
@@ -711,17 +780,18 @@ extern "C" int queue_prefill(gq_queue* q, const uint32_t* host_vals, uint64_t co
   // concurrent run, all-slow builds) the lanes take turns.
   const uint32_t serial = !q->fresh || (q->kind != GQ_LFQ && q->kind != GQ_LFQ_DIRECT && q->opts.enq_patience == GQ_PATIENCE_ZERO);
   q->fresh = false;
-  return dispatch(q, [&](auto& view) { return prefill_t(view, host_vals, count, st, serial); });
+  const uint32_t lanes = std::min(32u, q->max_threads);
+  return dispatch(q, [&](auto& view) { return prefill_t(view, host_vals, count, st, serial, lanes); });
 }
 
 template <class Q>
-static int drain_t(const Q& view, uint32_t* host_out, uint64_t max, uint64_t* n_out, cudaStream_t st) {
+static int drain_t(const Q& view, uint32_t* host_out, uint64_t max, uint64_t* n_out, cudaStream_t st, uint32_t lanes) {
   uint32_t* d_out = nullptr; uint64_t* d_n = nullptr;
   CU(cudaMalloc(&d_out, std::max<uint64_t>(max, 1) * 4));
   cudaError_t e = cudaMalloc(&d_n, 8);
   if (e != cudaSuccess) { cudaFree(d_out); return cuda_fail(e, "cudaMalloc"); }
   uint64_t n = 0;
-  drain_kernel<Q><<<1, 32, 0, st>>>(view, d_out, max, d_n);
+  drain_kernel<Q><<<1, 32, 0, st>>>(view, d_out, max, d_n, lanes);
   e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaMemcpyAsync(&n, d_n, 8, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -735,7 +805,8 @@ extern "C" int queue_drain(gq_queue* q, uint32_t* host_out, uint64_t max, uint64
   if (!q || !n_out || (!host_out && max)) return GQ_E_INVAL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   q->fresh = false;
-  return dispatch(q, [&](auto& view) { return drain_t(view, host_out, max, n_out, st); });
+  const uint32_t lanes = std::min(32u, q->max_threads);
+  return dispatch(q, [&](auto& view) { return drain_t(view, host_out, max, n_out, st, lanes); });
 }
 
 template <class Q>

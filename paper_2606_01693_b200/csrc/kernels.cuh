@@ -26,7 +26,9 @@ struct BenchParams {
   uint32_t jitter_ns, fail_backoff_ns;
   uint64_t value_base;
   const uint32_t* perm;        // physical -> logical thread id (role_layout 1), or nullptr
-  uint32_t fused, _pad;        // role_layout 2: mixed warps call the fused enqueue_or_dequeue (G-LFQ)
+  uint32_t tid_shift;          // > 0: payload = value_base + (thread << tid_shift | iter) (BASELINE.json configs[0]); 0: value_base + thread + iter * threads
+  uint32_t _pad;
+  uint32_t fused, converged;   // role_layout 2: mixed warps call the fused enqueue_or_dequeue (G-LFQ); converged: see gq_run_cfg
 };
 
 // the fused mixed-warp operation exists for G-LFQ (lfq.cuh); other kinds run the two calls
@@ -45,7 +47,75 @@ __device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
   return v;
 }
 
+// the unique payload of (logical thread, iteration)
+__device__ __forceinline__ uint32_t payload_of(const BenchParams& p, uint32_t ltid, uint32_t iter) {
+  return p.tid_shift ? (uint32_t)(p.value_base + ((uint64_t)ltid << p.tid_shift | iter))
+                     : (uint32_t)(p.value_base + ltid + (uint64_t)iter * p.threads);
+}
+
+// per-thread tallies of the benchmark loop
+struct Tally {
+  uint32_t succ_enq = 0, succ_deq = 0, full = 0, empty = 0, tot_enq = 0, tot_deq = 0, tot_full = 0, tot_empty = 0, fail_ns = 0;
+  uint64_t sum_enq = 0, sum_deq = 0, retries = 0;
+};
+__device__ __forceinline__ void fail_backoff(const BenchParams& p, Tally& a) {
+  if (p.fail_backoff_ns) { a.fail_ns = a.fail_ns ? min(a.fail_ns * 2, p.fail_backoff_ns) : 64; __nanosleep(a.fail_ns); }
+}
+// one enqueue / one dequeue of the benchmark loop, with its history record (kHist) and its tallies; returns the end stamp
+template <class Q, bool kHist, bool kWarpFaa>
+__device__ __forceinline__ uint64_t enq_step(const Q& q, thread_ctx& ctx, const BenchParams& p, uint32_t ltid, uint32_t iter,
+                                             uint64_t tw, uint64_t te, Tally& a, gq_hist_rec*& my) {
+  const uint32_t v = payload_of(p, ltid, iter);
+  uint64_t t_call = 0;
+  if (kHist) {
+    if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
+    t_call = globaltimer_ns();
+  }
+  const int s = enqueue<true, kWarpFaa>(q, ctx, v, &a.retries);
+  if (kHist) { __threadfence(); }               // effects performed before `end` is read (reading H1)
+  const uint64_t now = globaltimer_ns();
+  if (kHist) *my++ = gq_hist_rec{ltid, GQ_OP_ENQ, v, (uint32_t)s, 0u, 0u, t_call, now};
+  const bool in = now >= tw && now < te;
+  if (s == OK) { ++a.tot_enq; a.sum_enq += v; a.succ_enq += in; a.fail_ns = 0; }
+  else { ++a.tot_full; a.full += in; fail_backoff(p, a); }
+  return now;
+}
+template <class Q, bool kHist, bool kWarpFaa>
+__device__ __forceinline__ uint64_t deq_step(const Q& q, thread_ctx& ctx, const BenchParams& p, uint32_t ltid, uint32_t iter,
+                                             uint64_t tw, uint64_t te, Tally& a, gq_hist_rec*& my) {
+  uint32_t v = 0;
+  uint64_t t_call = 0;
+  if (kHist) {
+    if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0xc2b2ae35u) ^ (iter * 2u + 0x7654321u)) % (p.jitter_ns + 1));
+    t_call = globaltimer_ns();
+  }
+  const int s = dequeue<true, kWarpFaa>(q, ctx, &v, &a.retries);
+  if (kHist) { __threadfence(); }
+  const uint64_t now = globaltimer_ns();
+  if (kHist) *my++ = gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
+  const bool in = now >= tw && now < te;
+  if (s == OK) { ++a.tot_deq; a.sum_deq += v; a.succ_deq += in; a.fail_ns = 0; }
+  else { ++a.tot_empty; a.empty += in; fail_backoff(p, a); }
+  return now;
+}
+
+// End of one benchmark iteration.  cfg.converged: the lanes of a warp that run this loop start their next iteration
+// together (one ballot over the lanes still looping), which is how a lock-step wavefront runs the paper's kernels
+// (wave64) and what kUniform callers promise anyway; without it a warp that has split once (lanes leave a wait
+// loop at different polls) stays split for the rest of the launch and all its later WAVEFAA batches are partial.
+__device__ __forceinline__ bool loop_done(const BenchParams& p, uint32_t& act, bool done) {
+  if (p.converged) {
+    const uint32_t cont = __ballot_sync(act, !done);
+    act = cont;
+  }
+  return done;
+}
+
 // One kernel for both micro-benchmarks.  kHist: record {proc,op,arg,ret,call,end} per op.
+// Split mode ("each thread is a pure producer or a pure consumer"): the role is fixed for the whole launch, so
+// producers and consumers run two separate loops.  One shared loop with `if (producer) ... if (consumer) ...` inside
+// makes the two halves of a mixed warp wait for each other at the reconvergence point of every iteration, i.e. run
+// one after the other (measured: 27 Gops/s at p = 0.5 against 56 with homogeneous warps).
 template <class Q, bool kHist, bool kWarpFaa, bool kFused = false>
 __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint64_t* ctr, gq_hist_rec* hist) {
   cg::grid_group grid = cg::this_grid();
@@ -56,85 +126,58 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
   const bool fixed = p.ops_per_thread != 0;
   const uint64_t tw = fixed ? 0 : t0 + p.warmup_ns;
   const uint64_t te = fixed ? ~0ull : tw + p.duration_ns;
-
-  uint32_t succ_enq = 0, succ_deq = 0, full = 0, empty = 0, tot_enq = 0, tot_deq = 0, tot_full = 0, tot_empty = 0;
-  uint64_t sum_enq = 0, sum_deq = 0, retries = 0;
+  Tally a;
 
   if (tid < p.threads) {
     const uint32_t ltid = p.perm ? p.perm[tid] : tid;      // logical thread (roles, payloads, records); tid = physical
     thread_ctx ctx{ltid};
     ctx.help_peer = ltid + 1;
-    bool do_enq = true, do_deq = true;
-    if (p.mode == MODE_SPLIT) {
-      do_enq = (uint64_t)mix32(p.seed * 0x9e3779b9u + ltid) < p.prod_threshold;
-      do_deq = !do_enq;
-    }
-    const uint32_t per_iter = p.mode == MODE_SPLIT ? 1 : 2;
-    gq_hist_rec* my = kHist ? hist + (size_t)ltid * p.ops_per_thread * per_iter : nullptr;
-    uint32_t fail_ns = 0;
-    for (uint32_t iter = 0;; ++iter) {
-      uint64_t now = 0;
-      if (kFused && HasFused<Q>::value) {                   // split mode, mixed warps, one converged call per iteration
-        uint32_t v = (uint32_t)(p.value_base + ltid + (uint64_t)iter * p.threads);
+    const bool split = p.mode == MODE_SPLIT;
+    const bool do_enq = !split || (uint64_t)mix32(p.seed * 0x9e3779b9u + ltid) < p.prod_threshold;
+    gq_hist_rec* my = kHist ? hist + (size_t)ltid * p.ops_per_thread * (split ? 1 : 2) : nullptr;
+    if (kFused && HasFused<Q>::value) {                     // split mode, mixed warps, one converged call per iteration
+      for (uint32_t iter = 0;; ++iter) {
+        uint32_t v = payload_of(p, ltid, iter);
         const uint32_t v_in = v;
         uint64_t t_call = 0;
         if (kHist) {
           if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
           t_call = globaltimer_ns();
         }
-        const int s = fused_op<kWarpFaa>(q, ctx, do_enq, &v, &retries);
+        const int s = fused_op<kWarpFaa>(q, ctx, do_enq, &v, &a.retries);
         if (kHist) { __threadfence(); }
-        now = globaltimer_ns();
+        const uint64_t now = globaltimer_ns();
         if (kHist) *my++ = do_enq ? gq_hist_rec{ltid, GQ_OP_ENQ, v_in, (uint32_t)s, 0u, 0u, t_call, now}
                                   : gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
         const bool in = now >= tw && now < te;
-        if (do_enq) { if (s == OK) { ++tot_enq; sum_enq += v_in; succ_enq += in; } else { ++tot_full; full += in; } }
-        else        { if (s == OK) { ++tot_deq; sum_deq += v; succ_deq += in; } else { ++tot_empty; empty += in; } }
+        if (do_enq) { if (s == OK) { ++a.tot_enq; a.sum_enq += v_in; a.succ_enq += in; } else { ++a.tot_full; a.full += in; } }
+        else        { if (s == OK) { ++a.tot_deq; a.sum_deq += v; a.succ_deq += in; } else { ++a.tot_empty; a.empty += in; } }
         if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
-        continue;
       }
-      if (do_enq) {
-        const uint32_t v = (uint32_t)(p.value_base + ltid + (uint64_t)iter * p.threads);
-        uint64_t t_call = 0;
-        if (kHist) {
-          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
-          t_call = globaltimer_ns();
-        }
-        const int s = enqueue<true, kWarpFaa>(q, ctx, v, &retries);
-        if (kHist) { __threadfence(); }               // effects performed before `end` is read (reading H1)
-        now = globaltimer_ns();
-        if (kHist) *my++ = gq_hist_rec{ltid, GQ_OP_ENQ, v, (uint32_t)s, 0u, 0u, t_call, now};
-        const bool in = now >= tw && now < te;
-        if (s == OK) { ++tot_enq; sum_enq += v; succ_enq += in; fail_ns = 0; }
-        else {
-          ++tot_full; full += in;
-          if (p.fail_backoff_ns) { fail_ns = fail_ns ? min(fail_ns * 2, p.fail_backoff_ns) : 64; __nanosleep(fail_ns); }
-        }
+    } else if (!split) {
+      uint32_t act = __activemask();
+      for (uint32_t iter = 0;; ++iter) {
+        enq_step<Q, kHist, kWarpFaa>(q, ctx, p, ltid, iter, tw, te, a, my);
+        const uint64_t now = deq_step<Q, kHist, kWarpFaa>(q, ctx, p, ltid, iter, tw, te, a, my);
+        if (loop_done(p, act, fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te))) break;
       }
-      if (do_deq) {
-        uint32_t v = 0;
-        uint64_t t_call = 0;
-        if (kHist) {
-          if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0xc2b2ae35u) ^ (iter * 2u + 0x7654321u)) % (p.jitter_ns + 1));
-          t_call = globaltimer_ns();
-        }
-        const int s = dequeue<true, kWarpFaa>(q, ctx, &v, &retries);
-        if (kHist) { __threadfence(); }
-        now = globaltimer_ns();
-        if (kHist) *my++ = gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
-        const bool in = now >= tw && now < te;
-        if (s == OK) { ++tot_deq; sum_deq += v; succ_deq += in; fail_ns = 0; }
-        else {
-          ++tot_empty; empty += in;
-          if (p.fail_backoff_ns) { fail_ns = fail_ns ? min(fail_ns * 2, p.fail_backoff_ns) : 64; __nanosleep(fail_ns); }
-        }
+    } else if (do_enq) {
+      uint32_t act = __activemask();
+      for (uint32_t iter = 0;; ++iter) {
+        const uint64_t now = enq_step<Q, kHist, kWarpFaa>(q, ctx, p, ltid, iter, tw, te, a, my);
+        if (loop_done(p, act, fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te))) break;
       }
-      if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
+    } else {
+      uint32_t act = __activemask();
+      for (uint32_t iter = 0;; ++iter) {
+        const uint64_t now = deq_step<Q, kHist, kWarpFaa>(q, ctx, p, ltid, iter, tw, te, a, my);
+        if (loop_done(p, act, fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te))) break;
+      }
     }
   }
   __syncwarp();
   // warp-reduce, one atomic per warp per counter
-  uint64_t vals[11] = {succ_enq, succ_deq, full, empty, tot_enq, tot_deq, tot_full, tot_empty, sum_enq, sum_deq, retries};
+  uint64_t vals[11] = {a.succ_enq, a.succ_deq, a.full, a.empty, a.tot_enq, a.tot_deq, a.tot_full, a.tot_empty, a.sum_enq, a.sum_deq, a.retries};
 #pragma unroll
   for (int i = 0; i < 11; ++i) {
     const uint64_t s = warp_sum(vals[i]);
@@ -155,21 +198,23 @@ __device__ __forceinline__ void prefill_prepare(const DlfqView&) {}
 __device__ __forceinline__ void prefill_prepare(const WfqView&) {}
 __device__ __forceinline__ void prefill_prepare(const YmcView& q) { Ymc::advance(q.tail, ld_acquire(q.head)); }
 
+// `lanes` (<= 32, <= the queue's max_threads) lanes of the warp take part: thread_ctx::tid indexes per-thread records.
 template <class Q>
-__global__ void prefill_kernel(Q q, const uint32_t* vals, uint64_t count, uint64_t* n_ok, uint32_t serial) {
+__global__ void prefill_kernel(Q q, const uint32_t* vals, uint64_t count, uint64_t* n_ok, uint32_t serial, uint32_t lanes) {
   thread_ctx ctx{threadIdx.x};
   uint64_t ok = 0;
   if (threadIdx.x == 0) prefill_prepare(q);
   __syncwarp();
-  for (uint64_t base = 0; base < count; base += 32) {
+  for (uint64_t base = 0; base < count; base += lanes) {
     const uint64_t i = base + threadIdx.x;
+    const bool mine = threadIdx.x < lanes && i < count;
     if (serial) {
-      for (uint32_t l = 0; l < 32; ++l) {
-        if (threadIdx.x == l && i < count && enqueue<false, true>(q, ctx, vals[i]) == OK) ++ok;
+      for (uint32_t l = 0; l < lanes; ++l) {
+        if (threadIdx.x == l && mine && enqueue<false, true>(q, ctx, vals[i]) == OK) ++ok;
         __syncwarp();
       }
     } else {
-      if (i < count && enqueue<true, true>(q, ctx, vals[i]) == OK) ++ok;
+      if (mine && enqueue<true, true>(q, ctx, vals[i]) == OK) ++ok;
     }
     __syncwarp();
   }
@@ -182,11 +227,11 @@ __global__ void prefill_kernel(Q q, const uint32_t* vals, uint64_t count, uint64
 // cell), not in lane order: a lane that met a hole left by an abandoned ticket retries at a
 // later ticket.  Rounds are sequential, so ticket order across rounds is round order.
 template <class Q>
-__global__ void drain_kernel(Q q, uint32_t* out, uint64_t max, uint64_t* n_out) {
+__global__ void drain_kernel(Q q, uint32_t* out, uint64_t max, uint64_t* n_out, uint32_t lanes) {
   thread_ctx ctx{threadIdx.x};
   uint64_t n = 0;
   for (;;) {
-    const uint64_t want = max - n < 32 ? max - n : 32;
+    const uint64_t want = max - n < lanes ? max - n : lanes;
     if (want == 0) break;
     uint32_t v = 0;
     int s = EMPTY;

@@ -50,6 +50,8 @@ def main():
     ap.add_argument("--layout", type=int, default=0)
     ap.add_argument("--fail-backoff-ns", type=int, default=0)
     ap.add_argument("--pool-cells", type=int, default=0)
+    ap.add_argument("--converged", type=int, default=1, help="gq_run_cfg.converged (1 = what bench.py runs)")
+    ap.add_argument("--role-layout", type=int, default=0, help="split: gq_run_cfg.role_layout")
     a = ap.parse_args()
     if a.mode in ("bfs", "rt"):
         return run_app(a)
@@ -58,9 +60,9 @@ def main():
         if a.mode == "split":
             queue_prefill(q, np.arange(a.capacity // 2, dtype=np.uint32))
             r = run_split(q, threads=a.threads, ops_per_thread=a.ops, producer_fraction=a.producer_fraction, seed=1,
-                          value_base=a.capacity // 2, fail_backoff_ns=a.fail_backoff_ns)
+                          value_base=a.capacity // 2, fail_backoff_ns=a.fail_backoff_ns, converged=a.converged, role_layout=a.role_layout)
         else:
-            r = run_balanced(q, threads=a.threads, ops_per_thread=a.ops, fail_backoff_ns=a.fail_backoff_ns)
+            r = run_balanced(q, threads=a.threads, ops_per_thread=a.ops, fail_backoff_ns=a.fail_backoff_ns, converged=a.converged)
         left = queue_drain(q, a.capacity + 1)
     finally:
         queue_destroy(q)

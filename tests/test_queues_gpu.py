@@ -4,104 +4,39 @@ Several results are correct for a concurrent queue, so parity is membership: the
 history must be linearizable w.r.t. the sequential bounded FIFO,
 conserve items, and keep per-producer order (L336); single-threaded runs must equal the
 sequential model exactly, EMPTY/FULL included.  All integer: bit-exact.
+The checks themselves live in tests/queue_checks.py (tests/test_mutants_gpu.py runs the same
+functions on a deliberately broken build and expects them to fail).
 """
+import ctypes
+
 import numpy as np
 import pytest
 
 import oracle
 import paper_2606_01693_b200 as gq
+from queue_checks import (VARIANTS, check_balanced_fixed_ops, check_medium_history, check_prefill_drain, check_single_thread,
+                          check_tiny_balanced, check_tiny_split, check_token_protocol, check_warp_faa, conserve, is_direct,
+                          is_ymc, make, model_capacity, soft_slack, to_history, history_verdict, WGL_TALLY)
 
 pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
 
-Z = gq.GQ_PATIENCE_ZERO
-# (kind, extra gq_opts): the "-p0" variants force every operation onto the slow path, the only
-# way to give the helping code real coverage (reading W2 / Y8); "-p1" mixes fast and slow.
-VARIANTS = {
-    "G-LFQ": (gq.GQ_LFQ, {}),
-    "G-WFQ": (gq.GQ_WFQ, {}),
-    "G-WFQ-p0": (gq.GQ_WFQ, dict(enq_patience=Z, deq_patience=Z, help_delay=1)),
-    "G-WFQ-p1": (gq.GQ_WFQ, dict(enq_patience=1, deq_patience=1, help_delay=2)),
-    # G-WFQ-YMC: capacity does not throttle (reading Y3), so its model capacity is "unbounded";
-    # the pool is sized per test.  -p0: every enqueue takes the slow path, every dequeue makes one
-    # unparked attempt and then takes the slow path (reading Y8).
-    "G-WFQ-YMC": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22)),
-    "YMC-p0": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, enq_patience=Z, deq_patience=Z)),
-    "YMC-p1": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, enq_patience=1, deq_patience=1)),
-    # ablation builds (DESIGN.md section 3): "-listed" = the paper's listing order and fences (no D3-D6),
-    # "-eager" = polling-consumer mode used by the BFS / tracer drivers
-    "G-LFQ-listed": (gq.GQ_LFQ, dict(flags=gq.GQ_F_NO_OPT_CAS | gq.GQ_F_THR_FIRST | gq.GQ_F_NO_PAIRED_FAA | gq.GQ_F_FENCED_PAYLOAD)),
-    "G-LFQ-eager": (gq.GQ_LFQ, dict(flags=gq.GQ_F_EAGER_EMPTY)),
-    "G-WFQ-eager": (gq.GQ_WFQ, dict(flags=gq.GQ_F_EAGER_EMPTY)),
-    "YMC-eager": (gq.GQ_WFQ_YMC, dict(ymc_pool_cells=1 << 22, flags=gq.GQ_F_EAGER_EMPTY)),
-    # direct-payload single-ring ablation (include/gq/dlfq.cuh): capacity bound soft, at most n + k items
-    "G-LFQ-D": (gq.GQ_LFQ_DIRECT, {}),
-    "G-LFQ-D-eager": (gq.GQ_LFQ_DIRECT, dict(flags=gq.GQ_F_EAGER_EMPTY)),
-}
 KINDS = list(VARIANTS)          # every test below runs for each of these
-SMALL = KINDS                   # tiny / single-thread cases
 BIG = ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-D"]        # full-occupancy cases
 IDS = KINDS
-UNBOUNDED = 1 << 31
-
-
-def is_ymc(kind):
-    return VARIANTS[kind][0] == gq.GQ_WFQ_YMC
-
-
-def is_direct(kind):
-    return VARIANTS[kind][0] == gq.GQ_LFQ_DIRECT
-
-
-def soft_slack(kind, threads):
-    """G-LFQ-D may hold up to n + k items for a moment (dlfq.cuh); every other kind is exact."""
-    return threads if is_direct(kind) else 0
-
-
-def model_capacity(kind, capacity):
-    return UNBOUNDED if is_ymc(kind) else capacity
-
-
-def make(kind, capacity, **opts):
-    k, extra = VARIANTS[kind]
-    o = gq.gq_opts(**{**extra, **opts})
-    return gq.queue_create_ex(k, capacity, o)
-
-
-def to_history(recs):
-    return oracle.History(recs["proc"], recs["op"], recs["arg"], recs["ret_status"], recs["ret_val"],
-                          recs["call_ns"], recs["end_ns"])
 
 
 # ---------------------------------------------------------------- a1: WAVEFAA, Lemma III.1
 @pytest.mark.parametrize("threads,rounds,seed", [(32, 8, 1), (5000, 64, 2), (65536 + 17, 16, 3)])
 def test_warp_faa_tickets_distinct_and_contiguous(threads, rounds, seed):
-    t, final = gq.run_warp_faa_probe(threads, rounds, seed)
-    took = t[t != np.uint64(0xFFFFFFFFFFFFFFFF)]
-    assert final == len(took)
-    assert np.array_equal(np.sort(took), np.arange(len(took), dtype=np.uint64))
-    assert 0.3 < len(took) / t.size < 0.7          # the seeded divergence really split the warps
+    check_warp_faa(threads, rounds, seed)
 
 
 # ---------------------------------------------------------------- single thread == sequential model
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("capacity", [1, 2, 3, 128])
 def test_single_thread_equals_model(kind, capacity):
-    rng = np.random.default_rng(capacity)
-    n_ops = 6000
-    # biased phases so that both FULL and EMPTY are hit repeatedly
-    p = np.repeat(rng.choice([0.3, 0.5, 0.7], n_ops // 200), 200)
-    ops = (rng.random(n_ops) > p).astype(np.uint32)            # 0 ENQ, 1 DEQ
-    args = np.arange(1, n_ops + 1, dtype=np.uint32)
-    q = make(kind, capacity, max_threads=64)
-    try:
-        st, val = gq.queue_run_script(q, ops, args, tid=5)
-    finally:
-        gq.queue_destroy(q)
-    est, eval_ = oracle.fifo_replay(model_capacity(kind, capacity), ops, args)
-    assert np.array_equal(st, est)
-    ok_deq = (ops == 1) & (est == 0)
-    assert np.array_equal(val[ok_deq], eval_[ok_deq])
-    assert (est == oracle.ST_EMPTY).any() and (is_ymc(kind) or (est == oracle.ST_FULL).any())
+    check_single_thread(kind, capacity)
 
 
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
@@ -126,13 +61,9 @@ def test_fresh_fill_full_drain(kind):
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("capacity,count", [(1024, 1000), (1024, 77), (1024, 1024), (100, 0), (5, 5)])
 def test_prefill_drain_preserves_order(kind, capacity, count):
+    check_prefill_drain(kind, capacity, count)
     q = make(kind, capacity, max_threads=64)
     try:
-        vals = (np.arange(count, dtype=np.uint32) * 7 + 3)
-        gq.queue_prefill(q, vals)
-        out = gq.queue_drain(q, capacity + 10)
-        assert np.array_equal(out, vals)
-        assert len(gq.queue_drain(q, 10)) == 0
         if count:
             if not is_ymc(kind):
                 with pytest.raises(gq.GqError):            # does not fit: GQ_E_STATE
@@ -145,90 +76,68 @@ def test_prefill_drain_preserves_order(kind, capacity, count):
         gq.queue_destroy(q)
 
 
+def test_service_kernels_respect_small_max_threads():
+    # queues created for fewer than 32 threads: prefill / drain must not index per-thread records out of bounds
+    for kind in ("G-WFQ", "G-WFQ-p0", "G-WFQ-YMC", "YMC-p0", "G-LFQ"):
+        q = make(kind, 64, max_threads=4)
+        try:
+            vals = np.arange(40, dtype=np.uint32) + 5
+            gq.queue_prefill(q, vals)
+            assert np.array_equal(gq.queue_drain(q, 100), vals)
+            st, val = gq.queue_run_script(q, [0, 0, 1, 1, 1], [7, 8, 0, 0, 0], tid=3)
+            assert st.tolist() == [0, 0, 0, 0, gq.GQ_EMPTY] and val[2:4].tolist() == [7, 8]
+        finally:
+            gq.queue_destroy(q)
+
+
 # ---------------------------------------------------------------- BJ config 1: tiny history
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("seed", list(range(1, 9)))
 def test_tiny_balanced_history_is_linearizable(kind, seed):
-    q = make(kind, 128, max_threads=64, park_ns=2000)
-    try:
-        r = gq.run_balanced(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
-                            jitter_ns=200, seed=seed)
-        recs = gq.history_dump(q)
-        left = gq.queue_drain(q, 256)
-    finally:
-        gq.queue_destroy(q)
-    assert len(recs) == 2048 and r["blocks"] == 1
-    # reading H6: neither EMPTY nor FULL can legally occur in this configuration
-    assert r["tot_full"] == 0 and r["tot_empty"] == 0 and len(left) == 0
-    enq = recs[recs["op"] == 0]
-    assert sorted(enq["arg"].tolist()) == sorted(t + i * 64 for t in range(64) for i in range(16))
-    ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 128), relaxed_full=False, leftover=left)
-    assert ok, msg
+    check_tiny_balanced(kind, seed)
 
 
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("pf,seed", [(0.25, 1), (0.25, 2), (0.75, 3), (0.75, 4), (0.5, 5)])
 def test_tiny_split_history_with_empty_and_full(kind, pf, seed):
-    # reading H6: n = 16, 64 threads, 16 ops each: EMPTY frequent at 25 % producers, FULL at 75 %
-    q = make(kind, 16, max_threads=64, park_ns=1000)
-    try:
-        r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
-                         jitter_ns=200, seed=seed, producer_fraction=pf)
-        recs = gq.history_dump(q)
-        left = gq.queue_drain(q, 2048)
-    finally:
-        gq.queue_destroy(q)
-    assert len(recs) == 1024
-    assert is_ymc(kind) or len(left) <= 16 + soft_slack(kind, 64)
-    assert r["pool_exhausted"] == 0
+    r, _ = check_tiny_split(kind, pf, seed)
     if pf < 0.5:
         assert r["tot_empty"] > 0
     if pf > 0.5:
         assert r["tot_full"] > 0 or is_ymc(kind)
-    # exact search when it finishes; at 64-way overlap with many EMPTY/FULL returns it may not, and
-    # the verdict then rests on the exact OK/EMPTY characterisation + capacity bound + conservation
-    ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 16), relaxed_full=True, leftover=left,
-                                   max_steps=3_000_000, accept_unknown=True, soft_slack=soft_slack(kind, 64))
-    assert ok, msg
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("pf,seed", [(0.25, 11), (0.75, 12), (0.75, 13), (0.5, 14), (0.75, 15), (0.25, 16)])
+def test_small_split_history_exact_search_must_finish(kind, pf, seed):
+    # 16 threads x 8 operations on capacity 4: FULL- and EMPTY-heavy, and small enough that the exact WGL search against
+    # the bounded model with the relaxed FULL rule (reading G12) always finishes: no fallback to the polynomial checks
+    r, msg = check_tiny_split(kind, pf, seed, threads=16, ops=8, capacity=4, exact=True)
+    assert "linearizable" in msg
+    if pf > 0.5 and not is_ymc(kind) and not is_direct(kind):
+        assert r["tot_full"] > 0
 
 
 # ---------------------------------------------------------------- conservation at scale
-def _conserve(r, left, prefill_vals=()):
-    pre = np.asarray(prefill_vals, dtype=np.uint64)
-    assert r["tot_enq"] + len(pre) - r["tot_deq"] == len(left)
-    s_left = int(np.asarray(left, dtype=np.uint64).sum()) if len(left) else 0
-    assert (r["sum_enq"] + int(pre.sum()) - r["sum_deq"] - s_left) % 2**64 == 0
-
-
 @pytest.mark.parametrize("kind,threads,capacity", [(k, 2048 + 32 + 5, 1 << 12) for k in KINDS] + [(k, 0, 1 << 16) for k in BIG])
 def test_balanced_fixed_ops_conserves(kind, threads, capacity):
-    q = make(kind, capacity, **(dict(ymc_pool_cells=1 << 26) if is_ymc(kind) else {}))
-    try:
-        r = gq.run_balanced(q, threads=threads, ops_per_thread=32)
-        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else capacity + 1 + soft_slack(kind, 1 << 18))
-    finally:
-        gq.queue_destroy(q)
-    assert is_ymc(kind) or len(left) <= capacity + soft_slack(kind, r["threads_launched"])
-    assert r["pool_exhausted"] == 0
-    assert r["tot_enq"] + r["tot_full"] == r["threads_launched"] * 32
-    assert r["tot_deq"] + r["tot_empty"] == r["threads_launched"] * 32
-    _conserve(r, left)
-    assert len(set(left.tolist())) == len(left)
+    check_balanced_fixed_ops(kind, threads, capacity)
 
 
 @pytest.mark.parametrize("kind", BIG)
-def test_balanced_timed_full_occupancy(kind):
-    # BJ config 2 at full co-residency, shortened window; same launch configuration as bench.py
+@pytest.mark.parametrize("converged", [0, 1])
+def test_balanced_timed_full_occupancy(kind, converged):
+    # BJ config 2 at full co-residency, shortened window; same launch configuration as bench.py (converged = 1)
     q = make(kind, 1 << 16, **(dict(ymc_pool_cells=1 << 31) if is_ymc(kind) else {}))
     try:
-        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=20)
+        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=20, converged=converged)
         left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else (1 << 16) + 1 + soft_slack(kind, 1 << 18))
     finally:
         gq.queue_destroy(q)
     assert r["threads_launched"] == gq.queue_max_coresident_threads(VARIANTS[kind][0], 256)
     assert is_ymc(kind) or len(left) <= (1 << 16) + soft_slack(kind, r["threads_launched"])
     assert r["pool_exhausted"] == 0
-    _conserve(r, left)
+    conserve(r, left)
     assert r["succ_enq"] > 0 and r["succ_deq"] > 0
 
 
@@ -251,7 +160,7 @@ def test_split_timed_conserves(kind, pf):
         gq.queue_destroy(q)
     assert ymc or len(left) <= n + soft_slack(kind, r["threads_launched"])
     assert r["pool_exhausted"] == 0
-    _conserve(r, left, pre)
+    conserve(r, left, pre)
     # FIFO: what is left of the prefill comes out first and in order
     pre_left = left[left < n // 2]
     assert np.array_equal(pre_left, np.sort(pre_left)) and np.array_equal(left[: len(pre_left)], pre_left)
@@ -259,18 +168,7 @@ def test_split_timed_conserves(kind, pf):
 
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 def test_token_protocol_at_scale(kind):
-    # exactly once, no foreign token, per-producer monotone — 16384 threads
-    q = make(kind, 1 << 14, max_threads=16384)
-    try:
-        gq.run_split(q, threads=16384, ops_per_thread=24, record_history=1, producer_fraction=0.5, seed=11)
-        recs = gq.history_dump(q)
-        left = gq.queue_drain(q, 1 << 18)
-    finally:
-        gq.queue_destroy(q)
-    assert len(recs) == 16384 * 24
-    h = to_history(recs)
-    assert oracle.precheck(h) == ""
-    assert oracle.conservation(h, left) == ""
+    check_token_protocol(kind)
 
 
 def test_residency_is_enforced():
@@ -283,42 +181,117 @@ def test_residency_is_enforced():
         gq.queue_destroy(q)
 
 
+# ---------------------------------------------------------------- caller-owned storage (gq_opts.storage)
+@pytest.mark.parametrize("kind", ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-D"])
+def test_torch_owned_storage(kind):
+    # north_star: "PyTorch is used only for device memory and streams": the caller allocates queue_storage_bytes() with
+    # torch and the library only formats the block; BJ#1 through the checker on it, and nothing is written outside it
+    k, extra = VARIANTS[kind]
+    o = gq.gq_opts(**{**extra, "max_threads": 64, "park_ns": 8000})
+    nbytes = gq.queue_storage_bytes(k, 128, o)
+    assert nbytes > 0
+    guard = 4096
+    block = torch.full((nbytes + 2 * guard + 256,), 0x5A, dtype=torch.uint8, device="cuda")
+    base = (block.data_ptr() + guard + 255) // 256 * 256
+    o.storage, o.storage_bytes = base, nbytes
+    q = gq.queue_create_ex(k, 128, o)
+    try:
+        gq.run_balanced(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1, jitter_ns=200, seed=5)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, 256)
+        gq.queue_reset(q)
+        gq.queue_prefill(q, np.arange(100, dtype=np.uint32))
+        assert np.array_equal(gq.queue_drain(q, 200), np.arange(100, dtype=np.uint32))
+    finally:
+        gq.queue_destroy(q)
+    history_verdict(to_history(recs), model_capacity(kind, 128), False, left)
+    torch.cuda.synchronize()
+    host = block.cpu().numpy()
+    off = base - block.data_ptr()
+    assert (host[:off] == 0x5A).all() and (host[off + nbytes:] == 0x5A).all()       # the block survives queue_destroy, guards intact
+    assert (host[off:off + nbytes] != 0x5A).any()
+    o.storage_bytes = nbytes - 1
+    with pytest.raises(gq.GqError):
+        gq.queue_create_ex(k, 128, o)                                              # too small
+    o.storage, o.storage_bytes = base + 8, nbytes
+    with pytest.raises(gq.GqError):
+        gq.queue_create_ex(k, 128, o)                                              # not 256 B aligned
+
+
 # ---------------------------------------------------------------- G-WFQ slow path really runs
 @pytest.mark.parametrize("kind", ["G-WFQ-p0", "G-WFQ-p1"])
 def test_wfq_slow_path_is_exercised_and_counts_once(kind):
-    # Lemma III.7: each logical slow round advances Head/Tail exactly once.  With
-    # patience 0 and a quiescent end state every operation took the slow path.
+    # Lemma III.7: "each logical slow-path round advances Head or Tail exactly once ... Threshold decremented
+    # at most once".  With patience 0 every ring operation takes the slow path, so on a quiescent queue the Head counter has
+    # moved by exactly the number of global increments <c,NULL> -> <c+1,tid> that were won, and that number equals the number
+    # of INC bits cleared on local words, i.e. completed logical rounds, however many helpers worked on each round.  (Tail can
+    # also be raised by "catch up Tail", Alg. 1, so there the increments are a lower bound.)
     # parking and the probe switched off, so that fast attempts really fail and patience runs out
     q = make(kind, 256, max_threads=256, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
     try:
+        c0 = gq.queue_debug_counters(q)
         r = gq.run_split(q, threads=256, block_threads=64, ops_per_thread=32, producer_fraction=0.5, seed=3) \
             if kind.endswith("p1") else gq.run_balanced(q, threads=256, block_threads=64, ops_per_thread=32)
+        c1 = gq.queue_debug_counters(q)
         left = gq.queue_drain(q, 512)
     finally:
         gq.queue_destroy(q)
-    _conserve(r, left)
+    conserve(r, left)
     if kind.endswith("p0"):
         # 2 ring operations per successful queue op, 1 per FULL/EMPTY that reached the slow path
         assert r["slow_enq"] == r["tot_enq"] + r["tot_deq"]
         assert r["slow_deq"] >= r["tot_enq"] + r["tot_deq"]
+        assert r["helps"] > 0
+        for ring in ("aq", "fq"):
+            assert c1[f"{ring}_head_inc"] == c1[f"{ring}_head_clr"] > 0                      # one increment per logical round
+            assert c1[f"{ring}_tail_inc"] == c1[f"{ring}_tail_clr"] > 0
+            assert c1[f"{ring}_head"] - c0[f"{ring}_head"] == c1[f"{ring}_head_inc"]         # and nothing else moved Head
+            assert c1[f"{ring}_tail"] - c0[f"{ring}_tail"] >= c1[f"{ring}_tail_inc"]
+        # every dequeue round decremented Threshold once (Alg. 2), every successful enqueue reset it (Alg. 1)
+        assert c1["aq_threshold"] <= 3 * c1["N"] - 1 and c1["fq_threshold"] <= 3 * c1["N"] - 1
     else:
         assert r["slow_enq"] + r["slow_deq"] > 0
 
 
-@pytest.mark.parametrize("kind", ["YMC-p0", "YMC-p1"])
-def test_ymc_slow_paths_are_exercised(kind):
-    # parking and the probe off, so that dequeuers really overtake enqueuers and attempts fail
-    q = make(kind, 256, max_threads=256, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
+def test_wfq_note_field_survives_cycle_wrap():
+    # The Note field of a G-WFQ entry (Lemma III.8) is compared modulo 2^16 like Cycle.  64 threads on capacity 64:
+    # 2N = 128 slots, so 2^15 laps are 2^22 tickets; run well past that with patience 1 (fast and slow path mixed, no
+    # parking), so that slow-path enqueues meet slots in the upper half of the cycle space.  A Note left at its initial
+    # value would rule every slot out there and the slow enqueues would never finish (watchdog).
+    q = make("G-WFQ-p1", 64, max_threads=64, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
     try:
-        r = gq.run_split(q, threads=256, block_threads=64, ops_per_thread=64, producer_fraction=0.5, seed=3)
-        left = gq.queue_drain(q, 1 << 15)
+        tot_slow = 0
+        for rep in range(4):
+            r = gq.run_balanced(q, threads=64, block_threads=64, ops_per_thread=40000, value_base=rep * 64 * 40000)
+            c = gq.queue_debug_counters(q)
+            tot_slow += r["slow_enq"]
+            left = gq.queue_drain(q, 128)
+            conserve(r, left)
+        assert c["aq_tail"] > (1 << 23) and tot_slow > 0, (c, tot_slow)
     finally:
         gq.queue_destroy(q)
-    assert r["pool_exhausted"] == 0
-    _conserve(r, left)
-    if kind.endswith("p0"):
-        assert r["slow_enq"] == r["tot_enq"]         # every enqueue published a request
-    assert r["slow_enq"] > 0 and r["slow_deq"] > 0
+
+
+@pytest.mark.parametrize("kind", ["YMC-p0", "YMC-p1"])
+def test_ymc_slow_paths_are_exercised(kind):
+    # parking and the probe off, so that dequeuers really overtake enqueuers and attempts fail; whether a given run
+    # enters both slow paths depends on the interleaving, so several seeds share the burden
+    seen_enq = seen_deq = 0
+    for seed in range(3, 11):
+        q = make(kind, 256, max_threads=256, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
+        try:
+            r = gq.run_split(q, threads=256, block_threads=64, ops_per_thread=64, producer_fraction=0.5, seed=seed, jitter_ns=seed * 40)
+            left = gq.queue_drain(q, 1 << 15)
+        finally:
+            gq.queue_destroy(q)
+        assert r["pool_exhausted"] == 0
+        conserve(r, left)
+        if kind.endswith("p0"):
+            assert r["slow_enq"] == r["tot_enq"]         # every enqueue published a request
+        seen_enq += r["slow_enq"]; seen_deq += r["slow_deq"]
+        if seen_enq and seen_deq:
+            break
+    assert seen_enq > 0 and seen_deq > 0
 
 
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
@@ -343,17 +316,17 @@ def test_tiny_split_default_parking(kind, pf, seed):
 # ---------------------------------------------------------------- soak: past every 32-bit wrap
 @pytest.mark.parametrize("kind", ["G-LFQ", "G-WFQ"])
 def test_soak_past_the_ticket_tag_wrap(kind):
-    # G-LFQ's payload cells carry the low 32 bits of the AQ ticket (D6) and payload values are
+    # G-LFQ's payload cells carry the low 31 bits of the AQ ticket (D6) and payload values are
     # tid + iter*k mod 2^32: 600 ms at full co-residency is ~2.5e10 operations, i.e. more than 2^32 tickets
     # on each ring and more than 2^32 enqueues; G-WFQ's 16-bit cycle field wraps every 2^35 tickets.
     q = make(kind, 1 << 16)
     try:
-        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=600)
+        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=600, converged=1)
         left = gq.queue_drain(q, (1 << 16) + 1)
     finally:
         gq.queue_destroy(q)
     assert r["tot_enq"] + r["tot_deq"] > (1 << 33)
-    _conserve(r, left)
+    conserve(r, left)
 
 
 # ---------------------------------------------------------------- linearizability beyond the tiny config
@@ -363,30 +336,7 @@ def test_soak_past_the_ticket_tag_wrap(kind):
                          # and the empty-witness part of the bad-pattern check is not polynomial in those
                          [(k, 4096, 8, 512) for k in ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-listed"]])
 def test_medium_history_bad_pattern_check(kind, threads, ops, capacity):
-    # 65 536 recorded operations from 4096 threads (128 warps over several SMs), k <= n and k > n (index
-    # starvation: dequeuers of FQ park, D2).  Too large for the exact WGL search at this overlap, but for
-    # histories whose returns are all OK / EMPTY with unique values the bad-pattern characterisation
-    # (oracle.poly) is exact, so OK here IS a linearizability verdict for the unbounded-FIFO part; FULL
-    # returns (possible when k > n) are covered by the capacity lower bound and conservation.
-    q = make(kind, capacity, max_threads=threads, **(dict(ymc_pool_cells=1 << 24) if is_ymc(kind) else {}))
-    try:
-        r = gq.run_balanced(q, threads=threads, ops_per_thread=ops, record_history=1, jitter_ns=100, seed=11)
-        recs = gq.history_dump(q)
-        left = gq.queue_drain(q, capacity + threads + 1)
-    finally:
-        gq.queue_destroy(q)
-    assert len(recs) == threads * ops * 2
-    h = to_history(recs)
-    assert oracle.precheck(h) == ""
-    assert oracle.conservation(h, left) == ""
-    if r["tot_empty"] + r["tot_full"] >= 256:
-        # parking (D2) normally absorbs the index starvation; if this run returned many EMPTY / FULL anyway, the
-        # empty-witness part of the bad-pattern check would take minutes: keep the exact checks above and stop
-        pytest.skip("many EMPTY/FULL returns in this run: bad-pattern check skipped (not polynomial in those)")
-    pr, why = oracle.poly(h)
-    assert pr == oracle.LIN_OK, why
-    if not is_ymc(kind):
-        assert oracle.capacity_bound(h, capacity + soft_slack(kind, threads)) == ""
+    check_medium_history(kind, threads, ops, capacity, max_fail_returns=256)
 
 
 # ---------------------------------------------------------------- split with compacted roles
@@ -394,10 +344,10 @@ def test_medium_history_bad_pattern_check(kind, threads, ops, capacity):
 def test_split_role_layout_compact(kind):
     # role_layout = 1 (gq.h): the same seeded Bernoulli roles, but logical threads are placed so that warps are
     # homogeneous.  Same logical behaviour: tiny history through the checker, then BJ config 3 shape conserving.
-    q = make(kind, 16, max_threads=64, park_ns=1000)
+    q = make(kind, 16, max_threads=64, park_ns=4000)
     try:
-        r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1, jitter_ns=200, seed=3,
-                         producer_fraction=0.5, role_layout=1)
+        gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1, jitter_ns=200, seed=3,
+                     producer_fraction=0.5, role_layout=1)
         recs = gq.history_dump(q)
         left = gq.queue_drain(q, 2048)
     finally:
@@ -406,24 +356,14 @@ def test_split_role_layout_compact(kind):
     # a logical thread is a pure producer or a pure consumer, as drawn from the seed
     for t in range(64):
         assert len(set(recs["op"][recs["proc"] == t].tolist())) == 1
-    ok, msg = oracle.check_history(to_history(recs), model_capacity(kind, 16), relaxed_full=True, leftover=left,
-                                   max_steps=3_000_000, accept_unknown=True)
-    assert ok, msg
+    history_verdict(to_history(recs), model_capacity(kind, 16), True, left, max_steps=3_000_000, accept_unknown=True)
     if kind == "G-LFQ":
         # role_layout = 2: mixed warps through the fused gq::enqueue_or_dequeue (address-matched WAVEFAA inside a
-        # converged warp, reading G10); FULL- and EMPTY-heavy tiny histories through the checker
+        # converged warp, reading G10); FULL- and EMPTY-heavy histories small enough for the exact search
         for pf, seed in ((0.25, 1), (0.75, 2), (0.5, 3)):
-            q = make(kind, 16, max_threads=64, park_ns=1000)
-            try:
-                r = gq.run_split(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1, jitter_ns=200,
-                                 seed=seed, producer_fraction=pf, role_layout=2)
-                recs = gq.history_dump(q)
-                left = gq.queue_drain(q, 2048)
-            finally:
-                gq.queue_destroy(q)
-            ok, msg = oracle.check_history(to_history(recs), 16, relaxed_full=True, leftover=left, max_steps=3_000_000,
-                                           accept_unknown=True)
-            assert ok, msg
+            r, msg = check_tiny_split(kind, pf, seed, threads=32, ops=8, capacity=4, exact=True, role_layout=2)
+            assert "linearizable" in msg
+            check_tiny_split(kind, pf, seed, role_layout=2)
     else:
         q = make(kind, 16, max_threads=64)
         try:
@@ -438,8 +378,14 @@ def test_split_role_layout_compact(kind):
     try:
         gq.queue_prefill(q, pre)
         kw = dict(ops_per_thread=40) if ymc else dict(warmup_ms=2, duration_ms=10)
-        r = gq.run_split(q, threads=0, producer_fraction=0.5, seed=7, value_base=n // 2, role_layout=1, **kw)
+        r = gq.run_split(q, threads=0, producer_fraction=0.5, seed=7, value_base=n // 2, role_layout=1, converged=1, **kw)
         left = gq.queue_drain(q, (1 << 24) if ymc else n + 1)
     finally:
         gq.queue_destroy(q)
-    _conserve(r, left, pre)
+    conserve(r, left, pre)
+
+
+def test_zz_report_wgl_tally():
+    # how often the exact search decided the histories of this session (the rest fell back to the polynomial checks)
+    print(f"\nWGL exact search: finished on {WGL_TALLY['finished']} histories, undecided on {WGL_TALLY['unknown']}")
+    assert WGL_TALLY["finished"] > 0
