@@ -35,7 +35,12 @@ sys.path.insert(0, ROOT)
 
 CAPACITY = 1 << 16
 WARMUP_MS, DURATION_MS = 20.0, 100.0
-ALGO_BYTES_PER_OP = {"lfq": 40.5, "wfq": 37.0, "ymc": 12.0, "lfq_direct": 12.5}   # SURVEY §8(d) / DESIGN.md section 5
+# Algorithmic bytes per successful op: what the METHOD must move.  G-LFQ: 2 x 8 B slot
+# loads + 2 x 8 B slot atomics + 2 x 8/32 B hot atomics + one 4 B payload access = 36.5 B.  The 8 B ticket-tagged payload cell
+# of this implementation (D6) moves 4 B more per op: implementation overhead, reported separately.
+ALGO_BYTES_PER_OP = {"lfq": 36.5, "wfq": 37.0, "ymc": 12.0, "lfq_direct": 12.5}
+IMPL_EXTRA_BYTES_PER_OP = {"lfq": 4.0, "wfq": 4.0, "ymc": 4.0, "lfq_direct": 0.0}
+CEILING_WINDOWS, CEILING_MS = 5, 100.0     # every ceiling: median of 5 windows of 100 ms, spread reported
 KINDS = {"lfq": 0, "wfq": 1, "ymc": 2, "lfq_direct": 3}   # lfq_direct: ablation kind (include/gq/dlfq.cuh), sweep context only
 # G-WFQ-YMC never reuses a cell: a 120 ms run at ~25 Gops/s touches ~1.5 G cells, so
 # the timed runs get a 2^32-cell pool (64 GiB of the 180 GB HBM); the other kinds ignore the field.
@@ -275,11 +280,17 @@ def run_ours(args, rank, world, local_rank):
     value = ops_window_all / (args.steps * DURATION_MS * 1e-3) / 1e6
 
     # ---- ceilings at the same occupancy (rank 0, outside the timed region)
-    c1 = gq.run_faa_ceiling(1, threads=threads, warmup_ms=5, duration_ms=30)
-    c4 = gq.run_faa_ceiling(4, threads=threads, warmup_ms=5, duration_ms=30)
-    c1l = gq.run_faa_ceiling(1, per_lane=True, threads=threads, warmup_ms=5, duration_ms=30)
-    c1_tps = c1["succ_enq"] / c1["meas_seconds"]
-    c4_tps = c4["succ_enq"] / c4["meas_seconds"]
+    def ceiling(n_counters, per_lane=False):
+        """tickets/s of the bare FAA loop: median, min and max over CEILING_WINDOWS windows of CEILING_MS"""
+        xs = []
+        for _ in range(CEILING_WINDOWS):
+            r = gq.run_faa_ceiling(n_counters, per_lane=per_lane, threads=threads, warmup_ms=10, duration_ms=CEILING_MS)
+            xs.append(r["succ_enq"] / r["meas_seconds"])
+        return statistics.median(xs), min(xs), max(xs)
+
+    c1_tps, c1_min, c1_max = ceiling(1)
+    c4_tps, c4_min, c4_max = ceiling(4)
+    c1l_tps, _, _ = ceiling(1, per_lane=True)
     peaks, peak_src = measured_peaks()
     ops_per_s_kernel = (ops_all / len(results)) / (kernel_ms * 1e-3)      # whole launch / event duration
     algo_gbps = ops_per_s_kernel * ALGO_BYTES_PER_OP[args.kind] / 1e9
@@ -296,13 +307,42 @@ def run_ours(args, rank, world, local_rank):
                 "traffic_detail": traffic_detail, "traffic_note": "DRAM bytes of the committed ncu --set full capture of this kernel (fixed-op launch, "
                 "profiles/r1b_balanced_ncu_full.md): the rings are L2-resident, so DRAM sees the cold first touch only; L2 sector bytes per op beside it",
                 "kernel": "gqk::bench_kernel", "kernel_ms": kernel_ms,
-                "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run",
-                "c1_gtickets_s": c1_tps / 1e9, "c4_gtickets_s": c4_tps / 1e9,
-                "c1_per_lane_faa_gtickets_s": c1l["succ_enq"] / c1l["meas_seconds"] / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),
+                "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run (median of 5 x 100 ms)",
+                "c1_gtickets_s": c1_tps / 1e9, "c1_min_max": [c1_min / 1e9, c1_max / 1e9],
+                "c4_gtickets_s": c4_tps / 1e9, "c4_min_max": [c4_min / 1e9, c4_max / 1e9],
+                "ceiling_protocol": f"median of {CEILING_WINDOWS} windows of {CEILING_MS:.0f} ms (10 ms warm-up each)",
+                "c1_per_lane_faa_gtickets_s": c1l_tps / 1e9, "frac_of_c4_half": ops_per_s_kernel / (c4_tps / 2),
+                "frac_min_max": [ops_per_s_kernel / (2 * c1_max), ops_per_s_kernel / (2 * c1_min)],
+                "impl_extra_GBps": ops_per_s_kernel * IMPL_EXTRA_BYTES_PER_OP[args.kind] / 1e9,
                 "index_cycle_us": (2.0 * CAPACITY / ops_per_s_kernel * 1e6) if threads > CAPACITY else None,
                 "index_cycle_note": "k > n: the n indices each go FQ -> enqueuer -> AQ -> dequeuer -> FQ; ops/s = 2n / cycle (DESIGN.md section 5)",
                 "algorithmic_GBps": algo_gbps, "hbm_peak_GBps": peaks["hbm_gbs"], "hbm_peak_source": peak_src,
                 "hbm_frac": algo_gbps / peaks["hbm_gbs"]}
+
+    # ---- BJ#3 (split, p = 0.5, n = 2^20 prefilled to 2^19) against the same ceiling: the metric names "balanced, split"
+    roofline_split = None
+    try:
+        qs = gq.queue_create_ex(kind, 1 << 20, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
+        pre = np.arange(1 << 19, dtype=np.uint32)
+        runs = {}
+        for layout in (0, 1):
+            xs = []
+            for _ in range(3):
+                gq.queue_reset(qs)
+                gq.queue_prefill(qs, pre)
+                r = gq.run_split(qs, threads=threads, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=0.5, seed=1,
+                                 value_base=1 << 19, role_layout=layout)
+                xs.append((r["succ_enq"] + r["succ_deq"]) / r["meas_seconds"])
+            runs[layout] = xs
+        gq.queue_destroy(qs)
+        a0 = statistics.median(runs[0])
+        roofline_split = {"bound": "l2_atomic", "achieved": a0 / 1e9, "peak": 2 * c1_tps / 1e9, "unit": "Gop/s", "frac": a0 / (2 * c1_tps),
+                          "workload": "BJ#3 split, p = 0.5, capacity 2^20 prefilled 2^19, seeded Bernoulli roles (mixed warps), median of 3 x 100 ms",
+                          "runs_gops": [round(x / 1e9, 2) for x in runs[0]],
+                          "same_roles_on_homogeneous_warps_gops": [round(x / 1e9, 2) for x in runs[1]],
+                          "note": "mixed warps: every WAVEFAA batch holds about 16 tickets instead of 32 (DESIGN.md section 7)"}
+    except gq.GqError as e:
+        roofline_split = {"error": str(e)}
 
     # ---- thread sweep of BJ#2 and the producer-fraction sweep of BJ#3 (context, not timed)
     sweep = {}
@@ -397,7 +437,9 @@ def run_ours(args, rank, world, local_rank):
                 "d2h_bytes_per_step": 128 + 8 + 4 * (e2e_drained // args.steps),
                 "what": "queue_reset + run_balanced + queue_drain(host array) per step; all successful ops of the launch / host wall time"},
         "gpu_launches": args.steps * 3,      # per step: 2 format kernels (queue_reset) + 1 bench kernel
-        "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline, "sweep": sweep,
+        "clocks": clocks, "roofline": roofline, "roofline_split": roofline_split, "cpu_baseline": cpu_baseline, "sweep": sweep,
+        "reference_arm_note": "--impl reference runs the mutex oracle on ALL host threads (contended: a few Mops/s); its best point is 1 thread "
+                              "(cpu_baseline.value), so the driver's ours/reference ratio is several times larger than value / cpu_baseline.value",
         "conservation": "checked every e2e step: tot_enq - tot_deq == drained",
         # P:L359 protocol ("5 runs, median"): the timed steps one by one (rank 0's replica) and their median
         "per_step_mops": [round((r["succ_enq"] + r["succ_deq"]) / (DURATION_MS * 1e-3) / 1e6, 1) for r in results],

@@ -20,6 +20,10 @@
  *  - Ownership: queue_create allocates device memory owned by the handle until
  *    queue_destroy.  With gq_opts.storage the caller (e.g. torch) owns the device block and
  *    the library only formats it.  Caller buffers stay the caller's.
+ *    Every call returns only after its device work has completed, so work of two calls never overlaps, whatever
+ *    streams they name.  run_* / queue_run_script / the ceilings take no stream: they launch on the default stream.
+ *  - GQ_E_TIMEOUT (watchdog, GQ_WATCHDOG_S): the kernel is still running; its device buffers are deliberately not
+ *    freed (that would block on it).  The context is unusable until the process ends or the device is reset.
  *  - A handle is not safe for concurrent host calls.
  */
 #ifndef GQ_H_

@@ -31,11 +31,16 @@ enum : uint32_t {
   MUT_SLOW_NO_FIN = 8,      // G-WFQ: slow-path install does not finalise the request: item enqueued twice
   MUT_YMC_NO_CLAIM = 9,     // G-WFQ-YMC: fast dequeue takes the value without claiming the cell ([5] deq_fast): item dequeued twice
   MUT_LIFO_PAIR = 10,       // ring enqueue installs at slot t ^ 1 (P:L107 SLOT): neighbouring tickets swap their FIFO places
+  MUT_P2_ANY_SIDE = 11,     // G-WFQ: a phase-2 helper accepts a Tail-round record while helping on Head and vice versa (Alg. 2):
+                            // INC cleared on a local word whose round nobody won, two requests share one ticket, items lost
   MUT_COUNT
 };
 // self-contained (prim.cuh includes this file): plain volatile accesses are good enough for diagnostics
 __device__ __forceinline__ uint64_t dbg_ld(const void* p) { return p ? *static_cast<const volatile uint64_t*>(p) : 0; }
 __device__ __forceinline__ uint64_t dbg_now() { uint64_t t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory"); return t; }
+#ifndef GQ_DBG_SITES
+#undef GQ_TRACE_BY_INDEX
+#endif
 #ifdef GQ_MUTANTS
 static __device__ uint32_t g_mutation = 0;
 #define GQ_MUT(n) (::gq::detail::g_mutation == (uint32_t)(n))
@@ -53,9 +58,12 @@ static __device__ TraceRec g_trace[kTraceCap];
 #define GQ_SITE(i) atomicAdd(&::gq::detail::g_dbg[i], 1ull)
 #define GQ_COUNT(i, v) atomicAdd(&::gq::detail::g_dbg[i], (unsigned long long)(v))
 // first kTraceCap events only; once the ring is full the cost is one load of its own line
+#ifndef GQ_TRACE_MIN
+#define GQ_TRACE_MIN 0       /* -DGQ_TRACE_MIN=<n>: record only events whose site id (low byte) is >= n */
+#endif
 #define GQ_TRACE(site, r, ticket, entry, aux)                                                                    \
   do {                                                                                                           \
-    if (::gq::detail::dbg_ld(&::gq::detail::g_trace_n) < ::gq::detail::kTraceCap) {                               \
+    if (((site) & 0xffu) >= GQ_TRACE_MIN && ::gq::detail::dbg_ld(&::gq::detail::g_trace_n) < ::gq::detail::kTraceCap) { \
       const unsigned long long i_ = atomicAdd(&::gq::detail::g_trace_n, 1ull);                                   \
       if (i_ < ::gq::detail::kTraceCap)                                                                          \
         ::gq::detail::g_trace[i_] = ::gq::detail::TraceRec{::gq::detail::dbg_now(),                              \
@@ -64,6 +72,37 @@ static __device__ TraceRec g_trace[kTraceCap];
             (int64_t)::gq::detail::dbg_ld((r).threshold), (uint64_t)(aux)};                                      \
     }                                                                                                            \
   } while (0)
+// -DGQ_TRACE_BY_INDEX (with GQ_DBG_SITES): the trace ring is used as tables instead, for chasing the fate of one queue
+// index through FQ -> enqueuer -> AQ -> dequeuer -> FQ (this is how the shared phase-2 record of G-WFQ was found, D10):
+//   records [0, 65536/2)      the LAST event of each kind (8 kinds) per (ring, index < 4096): GQ_IDX_EVENT
+//   records [24576, 24576+2048*16)  the last 16 transitions of each G-WFQ local word of the AQ ring: GQ_L_EVENT
+// Both stop recording once event counter 70 is set (a check that wants the state frozen sets it with GQ_COUNT(70, 1)).
+#ifdef GQ_TRACE_BY_INDEX
+static __device__ unsigned int g_lcnt[2048];
+#define GQ_IDX_EVENT(kind, r, idx, ticket, entry, aux)                                                           \
+  do {                                                                                                           \
+    if (::gq::detail::dbg_ld(&::gq::detail::g_dbg[70]) == 0) {                                                    \
+      const uint32_t i_ = (((uint32_t)(idx) & 0xFFFu) + 4096u * (r).id) * 8u + (kind);                            \
+      if (i_ < 24576u)                                                                                           \
+        ::gq::detail::g_trace[i_] = ::gq::detail::TraceRec{::gq::detail::dbg_now(),                               \
+            (uint64_t)(kind) | ((uint64_t)(blockIdx.x * blockDim.x + threadIdx.x) << 32), (uint64_t)(ticket), (uint64_t)(entry), \
+            0, 0, 0, (uint64_t)(aux)};                                                                           \
+      ::gq::detail::g_trace_n = ::gq::detail::kTraceCap;                                                         \
+    }                                                                                                            \
+  } while (0)
+#define GQ_L_EVENT(r, target, kind, me, a, b)                                                                     \
+  do {                                                                                                           \
+    if ((r).id == 0 && ::gq::detail::dbg_ld(&::gq::detail::g_dbg[70]) == 0) {                                     \
+      const uint32_t t_ = (uint32_t)(target) & 2047u;                                                             \
+      const uint32_t n_ = atomicAdd(&::gq::detail::g_lcnt[t_], 1u);                                               \
+      ::gq::detail::g_trace[24576 + t_ * 16 + (n_ & 15u)] = ::gq::detail::TraceRec{::gq::detail::dbg_now(),       \
+          (uint64_t)(kind) | ((uint64_t)(me) << 32), (uint64_t)(a), (uint64_t)(b), n_, 0, 0, 0};                  \
+    }                                                                                                            \
+  } while (0)
+#else
+#define GQ_IDX_EVENT(kind, r, idx, ticket, entry, aux) ((void)0)
+#define GQ_L_EVENT(r, target, kind, me, a, b) ((void)0)
+#endif
 // Sampled latency probes: one thread in 2048 accumulates clock64 deltas per site.  `dep` is the value whose
 // arrival ends the interval: the compare makes the (in-order) warp wait for it before the clock is read.
 #define GQ_SAMPLED (((blockIdx.x * blockDim.x + threadIdx.x) & 2047u) == 0)
@@ -80,6 +119,8 @@ static __device__ TraceRec g_trace[kTraceCap];
 #define GQ_SITE(i) ((void)0)
 #define GQ_COUNT(i, v) ((void)0)
 #define GQ_TRACE(site, r, ticket, entry, aux) ((void)0)
+#define GQ_IDX_EVENT(kind, r, idx, ticket, entry, aux) ((void)0)
+#define GQ_L_EVENT(r, target, kind, me, a, b) ((void)0)
 #define GQ_TIC(var) ((void)0)
 #define GQ_TOC(site, var, dep) ((void)0)
 #endif

@@ -106,6 +106,9 @@ template <bool kUniform>
 __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 1) {
   uint32_t mask = __activemask();
   if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
+#ifdef GQ_DBG_SITES
+  if (kUniform && __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter)) != mask) GQ_COUNT(71, 1);   // kUniform promise broken
+#endif
   const uint32_t leader = __ffs(mask) - 1;
   const uint32_t rank = __popc(mask & lanemask_lt()) + (GQ_MUT(MUT_RANK_OFF_BY_ONE) ? 1u : 0u);
   uint64_t base = 0;

@@ -258,7 +258,7 @@ struct Ring {
       E = F::predicted(c);
       const uint64_t o = install_cas(sp, E, F::installed(E, c, x), flags);   // L153 on the predicted entry
       GQ_TOC(LAT_INSTALL_CAS + 5 * r.id, t1, o);
-      if (o == E) { reset_threshold(r, flags); return RING_OK; }      // L155
+      if (o == E) { GQ_IDX_EVENT(1, r, x, t, o, 0); reset_threshold(r, flags); return RING_OK; }      // L155
       E = o;                                                          // L148: the failed CAS read the slot
     } else {
       E = ld_relaxed(sp);                                             // L148
@@ -270,6 +270,7 @@ struct Ring {
         ok = counter(ld_relaxed(r.head)) <= t;
       }
       if (ok && install_cas(sp, E, F::installed(E, c, x), flags) == E) {   // L153: linearization point (L111)
+        GQ_IDX_EVENT(1, r, x, t, E, 1);
         reset_threshold(r, flags);                                    // L155
         return RING_OK;
       }
@@ -348,6 +349,7 @@ struct Ring {
       if (F::cycle(E) == c && !F::vacant(E)) {                        // L178
         GQ_TOC(LAT_SLOT_WAIT + 5 * r.id, t1, E);
         fin(r, h, j, E);                                              // G-WFQ: finalize an Enq=0 entry (W6)
+        GQ_IDX_EVENT(5, r, F::index(E), h, E, 0);
         red_or_relaxed(sp, F::kConsumeMask);                          // L180 CONSUME: linearization point
         *x = F::index(E);
         return RING_OK;                                               // L182

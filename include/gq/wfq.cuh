@@ -69,8 +69,13 @@ struct Wf {
   }
 
   // Help the phase-2 request named by ThrIdx u (Alg. 2): clear INC on the local word
-  // its record names.  Accepted only if the record's sequence pair matches and its counter is
-  // below the global counter c we saw next to u (a record of a later round has counter >= c).
+  // its record names.  Accepted only if the record's sequence pair matches, it is a record of THIS
+  // global word (a thread has one phase-2 record per ring, used for its Head rounds and its Tail
+  // rounds alike: Head may still name u after a Head round of u whose ThrIdx nobody has cleared yet,
+  // while u has since published a Tail round; its counter is a Tail counter, and clearing INC on
+  // that local tail would hand the request a ticket nobody drew), and its counter is below the
+  // global counter c we saw next to u (a record of a later round has counter >= c).
+  template <bool kDeq>
   __device__ static void help_phase2(const RingView& r, uint32_t u, uint64_t c, uint32_t me) {
     WfqRecord* p = rec(r, u);
     const uint64_t s2 = ld_acquire(&p->p2_seq2);
@@ -78,8 +83,10 @@ struct Wf {
     const uint64_t expect = ld_relaxed(&p->p2_expect);
     fence_acq_rel();
     if (ld_relaxed(&p->p2_seq1) != s2) return;
+    if (((target & 1) != 0) != kDeq && !GQ_MUT(MUT_P2_ANY_SIDE)) return;
     if ((expect >> S) >= c || !(expect & kINC)) return;
     if (cas_acq_rel(local_ptr(r, target), expect, expect & ~kINC) == expect) {
+      GQ_L_EVENT(r, target, 'P', me, expect, ((uint64_t)u << 44) | c);
       WfqRecord* mine = rec(r, me);
       ++((target & 1) ? mine->n_head_clr : mine->n_tail_clr);
     }
@@ -106,7 +113,7 @@ struct Wf {
         c = g >> S;
         const uint32_t u = (uint32_t)(g & kNull);
         if (u == kNull) { have = true; break; }
-        help_phase2(r, u, c, me);
+        help_phase2<kDeq>(r, u, c, me);
         if (cas_acq_rel(G, g, (c << S) | kNull) == g) { have = true; break; }
       }
       const uint64_t want = local_word(c, tag) | kINC;      // L258: synchronize L to c using INC
@@ -116,6 +123,7 @@ struct Wf {
         if (!(v & kINC)) return true;                       // round already completed by another helper
         c = v >> S;
       } else {
+        GQ_L_EVENT(r, target_id, 'S', me, v, want);
         v = want;
       }
       // L260: publish phase-2 record (L, c) under its sequence pair
@@ -130,6 +138,7 @@ struct Wf {
     }
     ++(kDeq ? mine->n_head_inc : mine->n_tail_inc);
     if (kDeq) faa_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)-1ll);   // L264-266
+    GQ_L_EVENT(r, target_id, 'W', me, v, c);
     if (cas_acq_rel(L, v, v & ~kINC) == v) ++(kDeq ? mine->n_head_clr : mine->n_tail_clr);   // L270: clear INC on L
     cas_acq_rel(G, ((c + 1) << S) | me, ((c + 1) << S) | kNull);         // L273: clear ThrIdx in G
     v &= ~kINC;
@@ -176,6 +185,7 @@ struct Wf {
         st_relaxed(r.owner + j, ((uint64_t)c << 32) | owner);
         const uint64_t N = F::installed_slow(E, c, x);        // <c, Safe 1, Enq 0, x>: linearization point
         if (cas_acq_rel(sp, E, N) != E) continue;
+        GQ_IDX_EVENT(3, r, x, T, E, v);
         if (GQ_MUT(MUT_SLOW_NO_FIN) && (T & 3) == 0) { cas_acq_rel(sp, N, N | F::kEnqBit); return false; }
         if (cas_acq_rel(L, v, v | kFIN) == v)                 // finalise the request ...
           cas_acq_rel(sp, N, N | F::kEnqBit);                 // ... and make the entry visible to fast dequeuers
@@ -183,6 +193,7 @@ struct Wf {
         return true;
       }
       if (F::cycle(E) == c && !F::vacant(E)) {                // installed by another helper of this request
+        GQ_IDX_EVENT(4, r, x, T, E, v);
         if (cas_acq_rel(L, v, v | kFIN) == v) cas_acq_rel(sp, E, E | F::kEnqBit);
         R::reset_threshold(r);
         return true;
@@ -305,6 +316,8 @@ struct Wf {
     st_release(&my->seq2, s);
     st_release32(&my->pending, 1u);
     ++my->n_slow_enq;
+    GQ_IDX_EVENT(2, r, x, t, 0, v0);
+    GQ_L_EVENT(r, (uint64_t)me << 1, 'I', me, v0, x);
     enqueue_slow(r, v0, x, me, tag, me);
     // The installer may be a helper that has not reached its Threshold reset yet while this
     // owner leaves through the FIN check: re-assert the reset (idempotent) so that the enqueue
@@ -360,6 +373,7 @@ struct Wf {
     const uint64_t E = ld_acquire(sp);
     if (F::cycle(E) == c && !F::vacant(E)) {
       fin(r, H, j, E);
+      GQ_IDX_EVENT(6, r, F::index(E), H, E, 0);
       red_or_relaxed(sp, F::kConsumeMask);                   // CONSUME: linearization point
       *x = F::index(E);
       return RING_OK;
@@ -393,6 +407,7 @@ __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32
     return FULL;
   }
   ctx.hungry &= ~2u;
+  GQ_IDX_EVENT(0, q.aq, idx, 0, 0, v);
   uint64_t* cell = q.data + idx;
   if (q.flags & kFencedPayload) {                                   // the paper's scheme: payload, then release-install
     st_relaxed(cell, (uint64_t)v);
@@ -426,6 +441,7 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq.tail);
   if (fast) w = cell_await(cell, w, ctx.last_ticket);               // tagged cell: wait for the store of THIS tenure of idx
   *out = (uint32_t)w;
+  GQ_IDX_EVENT(7, q.aq, idx, ctx.last_ticket, w, fast);
   const uint32_t fl = (q.flags & kFencedPayload) ? q.flags : (q.flags | kRelaxedInstall);
   Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, fl, paired, t);
   return OK;

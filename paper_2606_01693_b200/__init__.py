@@ -186,6 +186,13 @@ def queue_drain(q, max_items, stream=None):
     return out[: n.value].copy()
 
 
+def queue_device_view(q):
+    """The POD device view (gq::LfqView / WfqView / YmcView / DlfqView) as bytes, to hand to a user kernel by value."""
+    buf = C.create_string_buffer(512)
+    _chk(lib.queue_device_view(q, buf, 512), "queue_device_view")
+    return buf.raw
+
+
 def queue_debug_counters(q):
     """dict of the hot words of a quiescent queue (gq.h)."""
     out = np.zeros(16, np.uint64)

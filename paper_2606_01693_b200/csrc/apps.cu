@@ -240,6 +240,7 @@ int bfs_run_t(const uint64_t* d_rowptr, const uint32_t* d_col, uint32_t nv, uint
   if (e != cudaSuccess) { cleanup(); return e == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : gq_cuda_fail(e, "bfs launch"); }
   cudaEventRecord(e1, stream);
   rc = gq_wait_event(e1, gq_watchdog_slack_s());
+  if (rc == GQ_E_TIMEOUT) { qa.h = qb.h = nullptr; return rc; }   // kernel still running: freeing would block on it
   uint64_t c[B_COUNT] = {};
   float ms = 0;
   if (rc == 0) {
@@ -452,10 +453,9 @@ __global__ void __launch_bounds__(256) rt_kernel(Q q, RtArgs a) {
     if (lane == 0) s = dequeue<false, true>(q, ctx, &item);
     s = __shfl_sync(0xffffffffu, s, 0);
     if (s != OK) {
-      uint64_t pend = 0;
-      if (lane == 0) pend = ld_acquire(a.ctr + R_PENDING);
-      pend = __shfl_sync(0xffffffffu, pend, 0);
-      if (pend == 0 || ld_relaxed(a.ctr + R_ERROR) || pool_exhausted(q)) break;   // "until no work remains"
+      uint32_t stop = 0;                                          // decided by lane 0 for the whole warp
+      if (lane == 0) stop = ld_acquire(a.ctr + R_PENDING) == 0 || ld_relaxed(a.ctr + R_ERROR) || pool_exhausted(q);
+      if (__shfl_sync(0xffffffffu, stop, 0)) break;               // "until no work remains"
       idle_ns = idle_ns ? min(idle_ns * 2, 2000u) : 100u;
       __nanosleep(idle_ns);
       continue;
@@ -559,6 +559,7 @@ int rt_render_t(const gq_rt_scene& sc, float* d_rgb, gq_rt_stats* st_out, cudaSt
   rt_resolve_kernel<<<(npix + 255) / 256, 256, 0, stream>>>(a);
   cudaEventRecord(e1, stream);
   rc = gq_wait_event(e1, gq_watchdog_slack_s());
+  if (rc == GQ_E_TIMEOUT) { q.h = nullptr; return rc; }           // kernel still running: freeing would block on it
   uint64_t c[R_COUNT] = {};
   float ms = 0;
   if (rc == 0) {

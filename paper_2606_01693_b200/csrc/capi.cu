@@ -310,7 +310,7 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
     if (e != cudaSuccess) { delete q; return cuda_fail(e, "cudaMalloc(queue)"); }
     q->owns = true;
   }
-  cudaError_t e = cudaMalloc(&q->d_ctr, C_COUNT * sizeof(uint64_t));
+  cudaError_t e = cudaMalloc(&q->d_ctr, 2 * C_COUNT * sizeof(uint64_t));   // run counters + scratch of collect_stats
   if (e != cudaSuccess) { if (q->owns) cudaFree(q->base); delete q; return cuda_fail(e, "cudaMalloc(counters)"); }
   if (kind == GQ_LFQ_DIRECT) {
     q->dlfq.r = make_ring(q->base, L, L.off_aq, 0, 0);
@@ -470,8 +470,8 @@ __global__ void ymc_stats_kernel(YmcHandle* a, uint32_t n, uint64_t* out) {
 }
 static int collect_stats(gq_queue* q, gq_run_result* res) {
   if (q->kind == GQ_LFQ || q->kind == GQ_LFQ_DIRECT) return 0;
-  uint64_t* d = nullptr; uint64_t h[4] = {0, 0, 0, 0};
-  CU(cudaMalloc(&d, 32)); cudaMemset(d, 0, 32);
+  uint64_t* d = q->d_ctr + C_COUNT; uint64_t h[4] = {0, 0, 0, 0};
+  CU(cudaMemset(d, 0, 32));
   if (q->kind == GQ_WFQ)
     wfq_stats_kernel<<<(q->max_threads + 255) / 256, 256>>>(static_cast<WfqRecord*>(q->wfq.aq.rec), static_cast<WfqRecord*>(q->wfq.fq.rec), q->max_threads, d);
   else {
@@ -480,7 +480,6 @@ static int collect_stats(gq_queue* q, gq_run_result* res) {
   }
   cudaError_t e = cudaMemcpy(h, d, 32, cudaMemcpyDeviceToHost);
   if (e == cudaSuccess && h[3]) res->pool_exhausted = 1;
-  cudaFree(d);
   if (e != cudaSuccess) return cuda_fail(e, "stats");
   res->slow_enq = h[0]; res->slow_deq = h[1]; res->helps = h[2];
   return 0;
@@ -511,6 +510,22 @@ static int wait_event(cudaEvent_t ev, double budget_s) {
     std::this_thread::sleep_for(std::chrono::microseconds(200));
   }
 }
+
+// Events and scratch of one launch, released on every path out of the caller.  After a watchdog time-out the kernel is
+// still running and cudaFree / cudaEventDestroy would block on it: `abandon()` leaves them to the (stuck) context.
+struct LaunchRes {
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  void* scratch = nullptr;
+  bool abandoned = false;
+  int create() { CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1)); return 0; }
+  void abandon() { abandoned = true; }
+  ~LaunchRes() {
+    if (abandoned) return;
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (scratch) cudaFree(scratch);
+  }
+};
 
 struct Resolved { uint32_t threads, block, blocks, blocks_per_sm; };
 static int resolve_launch(int blocks_per_sm, const gq_run_cfg* cfg, uint32_t thread_cap, Resolved* r) {
@@ -641,17 +656,16 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   BenchParams p = make_params(cfg, r, mode);
   Q v = view;
   set_nthreads(v, r.threads);          // help ring = the launched threads (reading W7)
-  uint32_t* d_perm = nullptr;
+  LaunchRes lr;
   if (mode == MODE_SPLIT && cfg->role_layout == 1) {   // same seeded roles, producers first: homogeneous warps
     std::vector<uint32_t> perm; perm.reserve(r.threads);
     std::vector<uint32_t> cons; cons.reserve(r.threads);
     for (uint32_t t = 0; t < r.threads; ++t)
       ((uint64_t)gq::detail::mix32(p.seed * 0x9e3779b9u + t) < p.prod_threshold ? perm : cons).push_back(t);
     perm.insert(perm.end(), cons.begin(), cons.end());
-    CU(cudaMalloc(&d_perm, (size_t)r.threads * 4));
-    cudaError_t ce = cudaMemcpy(d_perm, perm.data(), (size_t)r.threads * 4, cudaMemcpyHostToDevice);
-    if (ce != cudaSuccess) { cudaFree(d_perm); return cuda_fail(ce, "memcpy(perm)"); }
-    p.perm = d_perm;
+    CU(cudaMalloc(&lr.scratch, (size_t)r.threads * 4));
+    CU(cudaMemcpy(lr.scratch, perm.data(), (size_t)r.threads * 4, cudaMemcpyHostToDevice));
+    p.perm = static_cast<const uint32_t*>(lr.scratch);
   } else if (mode == MODE_SPLIT && cfg->role_layout == 2) {
     p.fused = 1;
   } else if (cfg->role_layout != 0 && mode == MODE_SPLIT) {
@@ -659,16 +673,15 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   }
   uint64_t* ctr = q->d_ctr; gq_hist_rec* h = q->d_hist;
   void* args[] = {&v, &p, &ctr, &h};
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
-  CU(cudaEventRecord(e0, nullptr));
+  rc = lr.create();
+  if (rc) return rc;
+  CU(cudaEventRecord(lr.e0, nullptr));
   cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
-  if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); if (d_perm) cudaFree(d_perm); return le == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : cuda_fail(le, "launch"); }
-  CU(cudaEventRecord(e1, nullptr));
-  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
-  if (rc == 0) rc = finish_run(q->d_ctr, e0, e1, cfg, r, res);
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  if (d_perm) cudaFree(d_perm);
+  if (le != cudaSuccess) return le == cudaErrorCooperativeLaunchTooLarge ? GQ_E_RESIDENCY : cuda_fail(le, "launch");
+  CU(cudaEventRecord(lr.e1, nullptr));
+  rc = wait_event(lr.e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
+  if (rc == GQ_E_TIMEOUT) { lr.abandon(); return rc; }
+  if (rc == 0) rc = finish_run(q->d_ctr, lr.e0, lr.e1, cfg, r, res);
   if (rc == 0) report_stuck();
   if (rc == 0) rc = collect_stats(q, res);
   if (rc == 0 && res->pool_exhausted) return GQ_E_POOL;
@@ -695,15 +708,16 @@ static int run_ceiling(K kernel, const gq_run_cfg* cfg, gq_run_result* res, uint
   if (rc) return rc;
   BenchParams p = make_params(cfg, r, MODE_BALANCED);
   args[2] = &p;
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
-  CU(cudaEventRecord(e0, nullptr));
+  LaunchRes lr;
+  rc = lr.create();
+  if (rc) return rc;
+  CU(cudaEventRecord(lr.e0, nullptr));
   cudaError_t le = cudaLaunchCooperativeKernel((void*)kernel, dim3(r.blocks), dim3(r.block), args, 0, nullptr);
-  if (le != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return cuda_fail(le, "launch"); }
-  CU(cudaEventRecord(e1, nullptr));
-  rc = wait_event(e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
-  if (rc == 0) rc = finish_run(d_ctr, e0, e1, cfg, r, res);
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (le != cudaSuccess) return cuda_fail(le, "launch");
+  CU(cudaEventRecord(lr.e1, nullptr));
+  rc = wait_event(lr.e1, (cfg->warmup_ms + cfg->duration_ms) * 1e-3 + watchdog_slack_s());
+  if (rc == GQ_E_TIMEOUT) { lr.abandon(); return rc; }
+  if (rc == 0) rc = finish_run(d_ctr, lr.e0, lr.e1, cfg, r, res);
   return rc;
 }
 
@@ -720,7 +734,7 @@ extern "C" int run_faa_ceiling(const gq_run_cfg* cfg, uint32_t n_counters, gq_ru
   void* args[4] = {&d_counters, &n_counters, nullptr, &d_ctr};
   int rc = per_lane ? run_ceiling(faa_ceiling_kernel<false>, cfg, res, d_ctr, args)
                     : run_ceiling(faa_ceiling_kernel<true>, cfg, res, d_ctr, args);
-  cudaFree(d_counters); cudaFree(d_ctr);
+  if (rc != GQ_E_TIMEOUT) { cudaFree(d_counters); cudaFree(d_ctr); }
   return rc;
 }
 
@@ -734,7 +748,7 @@ extern "C" int run_slot_atomic_ceiling(const gq_run_cfg* cfg, uint64_t slots, gq
   cudaMemset(d_buf, 0, slots * 8); cudaMemset(d_ctr, 0, C_COUNT * 8);
   void* args[4] = {&d_buf, &slots, nullptr, &d_ctr};
   int rc = run_ceiling(slot_ceiling_kernel, cfg, res, d_ctr, args);
-  cudaFree(d_buf); cudaFree(d_ctr);
+  if (rc != GQ_E_TIMEOUT) { cudaFree(d_buf); cudaFree(d_ctr); }
   return rc;
 }
 

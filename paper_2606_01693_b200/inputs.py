@@ -1,7 +1,8 @@
 """Seeded synthetic inputs for the application drivers (BASELINE.json configs 4 and 5).
 
-Input tooling only: numpy, none of the method's arithmetic, imported neither by the CUDA
-library nor by the CPU checker.  Tests and bench.py build the arrays here and hand the same arrays
+Input tooling only: numpy (plus a torch transcription of the graph recipe, so that the scale-22 graph of
+config 4 can be generated on the GPU box in seconds instead of minutes), none of the method's arithmetic,
+imported neither by the CUDA library nor by the CPU checker.  Tests and bench.py build the arrays here and hand the same arrays
 to both sides.  They stand in for the paper's SuiteSparse graphs (Table IV,
 L428-440) and its two scenes (L366, L384), which are not available.
 """
@@ -68,6 +69,58 @@ def rmat_csr(scale, edge_factor=16, seed=1):
     rowptr, col = csr_undirected(nv, src, dst)
     deg = np.diff(rowptr.astype(np.int64))
     nonisolated = np.flatnonzero(deg > 0)
+    source = int(nonisolated[seed % len(nonisolated)])
+    return rowptr, col, source
+
+
+# ---- the same recipe with torch ops (any device): bit-identical arrays, tests/test_inputs.py compares the two on CPU.
+# torch has no uint64 arithmetic: int64 with wrapping multiplication, logical shifts written out.
+def _i64(c):
+    return c - (1 << 64) if c >= (1 << 63) else c
+
+
+def _lsr(x, s):
+    return (x >> s) & ((1 << (64 - s)) - 1)
+
+
+def _splitmix64_torch(x):
+    x = x + _i64(0x9E3779B97F4A7C15)
+    x = (x ^ _lsr(x, 30)) * _i64(0xBF58476D1CE4E5B9)
+    x = (x ^ _lsr(x, 27)) * _i64(0x94D049BB133111EB)
+    return x ^ _lsr(x, 31)
+
+
+def rmat_csr_torch(scale, edge_factor=16, seed=1, device="cpu", a=0.57, b=0.19, c=0.19, chunk=1 << 24):
+    """rmat_csr() computed with torch on `device`.  Returns (rowptr int64[nv+1], col int32[], source) as torch tensors
+    on that device; values equal those of rmat_csr (rowptr uint64, col uint32) element for element."""
+    import torch
+    nv = 1 << scale
+    n_edges = edge_factor << scale
+    key = int(_splitmix64(np.array([seed], np.uint64))[0])
+    key = _i64(key)
+    keys = []
+    for lo in range(0, n_edges, chunk):
+        hi = min(lo + chunk, n_edges)
+        e = torch.arange(lo, hi, dtype=torch.int64, device=device)
+        u = torch.zeros(hi - lo, dtype=torch.int64, device=device)
+        v = torch.zeros(hi - lo, dtype=torch.int64, device=device)
+        for level in range(scale):
+            h = _splitmix64_torch((e * 64 + level) ^ key)
+            r = _lsr(h, 11).to(torch.float64) * (1.0 / (1 << 53))
+            ubit = r >= a + b
+            vbit = ((r >= a) & (r < a + b)) | (r >= a + b + c)
+            u = (u << 1) | ubit.to(torch.int64)
+            v = (v << 1) | vbit.to(torch.int64)
+        keep = u != v
+        u, v = u[keep], v[keep]
+        keys.append(torch.unique(torch.cat([(u << 32) | v, (v << 32) | u])))
+    keys = torch.unique(torch.cat(keys))
+    rows = keys >> 32
+    col = (keys & 0xFFFFFFFF).to(torch.int32)
+    counts = torch.bincount(rows, minlength=nv)
+    rowptr = torch.zeros(nv + 1, dtype=torch.int64, device=device)
+    rowptr[1:] = torch.cumsum(counts, 0)
+    nonisolated = torch.nonzero(counts > 0).flatten()
     source = int(nonisolated[seed % len(nonisolated)])
     return rowptr, col, source
 

@@ -153,7 +153,7 @@ def check_tiny_split(kind, pf, seed, threads=64, ops=16, capacity=16, exact=Fals
     extra = dict(flags=VARIANTS[kind][1].get("flags", 0) | gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE) if park_flags else {}
     q = make(kind, capacity, max_threads=max(threads, 32), park_ns=4000, **extra)
     try:
-        r = gq.run_split(q, threads=threads, block_threads=min(threads, 64), ops_per_thread=ops, record_history=1,
+        r = gq.run_split(q, threads=threads, block_threads=max(32, min(threads, 64)), ops_per_thread=ops, record_history=1,
                          jitter_ns=200, seed=seed, producer_fraction=pf, **run_kw)
         recs = gq.history_dump(q)
         left = gq.queue_drain(q, 2048)
@@ -230,3 +230,33 @@ def check_medium_history(kind, threads, ops, capacity, max_fail_returns=4096):
         msg = oracle.capacity_bound(h, capacity + soft_slack(kind, threads))
         assert msg == "", msg
     return f"{r['tot_empty']} EMPTY, {r['tot_full']} FULL"
+
+
+# ---------------------------------------------------------------- fast and slow paths mixed, long, on a tiny ring
+def check_slow_fast_mix_stress(kind, reps=6, threads=64, capacity=64, ops=40000):
+    """Producers and consumers in separate warps (role_layout 1) on a ring as small as the thread count, no parking and no
+    probe, patience 1: consumers that poll the empty ring invalidate slots under the producers' feet, so a large share of
+    the operations goes through the helping slow paths while the rest stays on the fast path, for millions of tickets and
+    thousands of laps.  Checked per launch: items and payload checksums are conserved, and no queue index is lost (a queue
+    that ends a launch full must still hold `capacity` items).  This is the run that exposed the shared phase-2 record of
+    G-WFQ (D10): a request was handed a ticket nobody drew, and items and indices vanished."""
+    q = make(kind, capacity, max_threads=threads, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE,
+             **(dict(ymc_pool_cells=1 << 26) if is_ymc(kind) else {}))
+    slow = 0
+    try:
+        for rep in range(reps):
+            r = gq.run_split(q, threads=threads, block_threads=32, ops_per_thread=ops, producer_fraction=0.5, seed=7 + rep,
+                             role_layout=1, value_base=rep * threads * ops)
+            assert r["pool_exhausted"] == 0
+            slow += r["slow_enq"] + r["slow_deq"]
+            left = gq.queue_drain(q, (threads * ops + 1) if is_ymc(kind) else (capacity + threads + 1))   # YMC is unbounded
+            conserve(r, left)
+            if not is_ymc(kind):
+                # fill it up single-handedly: exactly `capacity` enqueues must succeed, i.e. every index is still in circulation
+                st, _ = gq.queue_run_script(q, np.zeros(capacity + 2, np.uint32), np.arange(capacity + 2, dtype=np.uint32), tid=1)
+                assert (st == 0).sum() == capacity, f"launch {rep}: only {(st == 0).sum()} of {capacity} indices left in circulation"
+                assert np.array_equal(gq.queue_drain(q, capacity + 1), np.arange(capacity, dtype=np.uint32))
+    finally:
+        gq.queue_destroy(q)
+    assert slow > 0, "the slow paths were never entered"
+    return f"{slow} slow-path operations"

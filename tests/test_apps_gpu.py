@@ -79,6 +79,25 @@ def test_bfs_rmat_bit_exact(kind, scale, threads):
     assert st["levels"] >= 3
 
 
+def test_bfs_config4_scale22_bit_exact():
+    # BASELINE.json configs[3] at its stated size: R-MAT scale 22, edge factor 16.  The graph comes from the torch
+    # transcription of the recipe (tests/test_inputs.py: same arrays as the numpy one), generated on the GPU in seconds.
+    # The frontier queues have capacity 2^22: rings of 64 MiB, which take the slot-prefetch path of rings too large for L2.
+    rowptr, col, src = inputs.rmat_csr_torch(22, 16, seed=1, device="cuda")
+    nv = len(rowptr) - 1
+    assert nv == 4194304
+    h_rowptr, h_col = rowptr.cpu().numpy().astype(np.uint64), col.cpu().numpy().view(np.uint32)
+    exp, exp_edges = oracle.bfs(h_rowptr, h_col, src)
+    d_dist = torch.empty(nv, dtype=torch.int32, device="cuda")
+    for kind, name in zip(KINDS, IDS):
+        d_dist.fill_(-7)
+        st = gq.bfs_run(kind, rowptr.data_ptr(), col.data_ptr(), nv, src, d_dist.data_ptr())
+        torch.cuda.synchronize()
+        assert np.array_equal(d_dist.cpu().numpy(), exp), name                 # bit-exact
+        assert st["edges_scanned"] == exp_edges and st["vertices_visited"] == int((exp >= 0).sum()), name
+        assert st["queue_ops"] == 2 * st["vertices_visited"], name
+
+
 def test_bfs_rejects_bad_arguments():
     rowptr, col = csr(4, [(0, 1), (1, 2)])
     with pytest.raises(gq.GqError):

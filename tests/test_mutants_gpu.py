@@ -27,6 +27,7 @@ MUTANTS = {
     8: ("G-WFQ slow-path install without FIN: item enqueued twice", ["G-WFQ-p0"]),
     9: ("G-WFQ-YMC fast dequeue without claiming the cell", ["YMC-p1", "G-WFQ-YMC"]),
     10: ("ring enqueue installs at slot t ^ 1", ["G-LFQ", "G-WFQ"]),
+    11: ("G-WFQ phase-2 helper accepts a record of the other global word (the bug of DESIGN.md D10)", ["G-WFQ-p1"]),
 }
 
 
@@ -43,9 +44,12 @@ def battery(kind):
     steps += [(f"tiny_split[{pf},{s}]", lambda pf=pf, s=s: qc.check_tiny_split(kind, pf, s)) for pf, s in ((0.25, 1), (0.75, 3), (0.5, 5))]
     steps += [("no_parking_split", lambda: qc.check_tiny_split(kind, 0.5, 21, threads=64, ops=64, capacity=8, park_flags=True)),
               ("fixed_ops", lambda: qc.check_balanced_fixed_ops(kind, 2048 + 37, 1 << 12)),
-              ("medium[k<=n]", lambda: qc.check_medium_history(kind, 4096, 8, 8192, max_fail_returns=256)),
-              ("medium[k>n]", lambda: qc.check_medium_history(kind, 4096, 8, 512, max_fail_returns=256)),
-              ("token_protocol", lambda: qc.check_token_protocol(kind, threads=4096, ops=24))]
+              ("medium[k<=n]", lambda: qc.check_medium_history(kind, 4096, 8, 8192, max_fail_returns=256))]
+    if "-p" not in kind:        # k > n: only the fast paths park (D2); the all-slow builds answer index starvation with FULL / EMPTY
+        steps += [("medium[k>n]", lambda: qc.check_medium_history(kind, 4096, 8, 512, max_fail_returns=256))]
+    steps += [("token_protocol", lambda: qc.check_token_protocol(kind, threads=4096, ops=24))]
+    if kind.endswith("-p1"):
+        steps += [("slow_fast_mix_stress", lambda: qc.check_slow_fast_mix_stress(kind, reps=24))]
     for name, fn in steps:
         try:
             fn()
@@ -64,7 +68,7 @@ def mutants():
         gq.gq_set_mutation(0)
 
 
-@pytest.mark.parametrize("kind", ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-WFQ-p0", "YMC-p1"])
+@pytest.mark.parametrize("kind", ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-WFQ-p0", "G-WFQ-p1", "YMC-p1"])
 def test_instrumented_build_without_fault_passes(mutants, kind):
     gq.gq_set_mutation(0)
     assert battery(kind) is None

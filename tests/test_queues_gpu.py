@@ -15,7 +15,7 @@ import pytest
 import oracle
 import paper_2606_01693_b200 as gq
 from queue_checks import (VARIANTS, check_balanced_fixed_ops, check_medium_history, check_prefill_drain, check_single_thread,
-                          check_tiny_balanced, check_tiny_split, check_token_protocol, check_warp_faa, conserve, is_direct,
+                          check_tiny_balanced, check_tiny_split, check_token_protocol, check_warp_faa, check_slow_fast_mix_stress, conserve, is_direct,
                           is_ymc, make, model_capacity, soft_slack, to_history, history_verdict, WGL_TALLY)
 
 pytestmark = pytest.mark.gpu
@@ -66,8 +66,10 @@ def test_prefill_drain_preserves_order(kind, capacity, count):
     try:
         if count:
             if not is_ymc(kind):
-                with pytest.raises(gq.GqError):            # does not fit: GQ_E_STATE
-                    gq.queue_prefill(q, np.arange(capacity + 1, dtype=np.uint32))
+                # does not fit: GQ_E_STATE.  G-LFQ-D's bound is soft (G12'): the 32 lanes of one prefill round pass its FULL
+                # test together, so only the round after the overshoot is refused
+                with pytest.raises(gq.GqError):
+                    gq.queue_prefill(q, np.arange(capacity + (33 if is_direct(kind) else 1), dtype=np.uint32))
             else:
                 gq.queue_prefill(q, np.arange(7, dtype=np.uint32))
             gq.queue_reset(q)
@@ -258,18 +260,44 @@ def test_wfq_note_field_survives_cycle_wrap():
     # 2N = 128 slots, so 2^15 laps are 2^22 tickets; run well past that with patience 1 (fast and slow path mixed, no
     # parking), so that slow-path enqueues meet slots in the upper half of the cycle space.  A Note left at its initial
     # value would rule every slot out there and the slow enqueues would never finish (watchdog).
+    # Producers and consumers sit in different warps (role_layout 1) so that they really run side by side: consumers that
+    # poll the empty ring invalidate the slots under the producers' feet, whose single fast attempt then fails.
     q = make("G-WFQ-p1", 64, max_threads=64, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
     try:
-        tot_slow = 0
-        for rep in range(4):
-            r = gq.run_balanced(q, threads=64, block_threads=64, ops_per_thread=40000, value_base=rep * 64 * 40000)
+        slow_upper = 0          # slow-path enqueues performed while AQ tickets were in the upper half of the cycle space and beyond
+        c = gq.queue_debug_counters(q)
+        for rep in range(64):
+            upper = c["aq_tail"] >= (1 << 22)
+            r = gq.run_split(q, threads=64, block_threads=32, ops_per_thread=40000, producer_fraction=0.5, seed=7 + rep,
+                             role_layout=1, value_base=rep * 64 * 40000)
             c = gq.queue_debug_counters(q)
-            tot_slow += r["slow_enq"]
+            if upper:
+                slow_upper += r["slow_enq"]
             left = gq.queue_drain(q, 128)
             conserve(r, left)
-        assert c["aq_tail"] > (1 << 23) and tot_slow > 0, (c, tot_slow)
+            if c["aq_tail"] > (1 << 23) + (1 << 22) and slow_upper > 0:
+                break
+        assert c["aq_tail"] > (1 << 23) and slow_upper > 0, (c, slow_upper)
     finally:
         gq.queue_destroy(q)
+
+
+@pytest.mark.parametrize("kind", ["G-WFQ-p1", "YMC-p1", "G-LFQ"])
+def test_slow_and_fast_paths_mixed_for_millions_of_tickets(kind):
+    print(check_slow_fast_mix_stress(kind, reps=12) if kind != "G-LFQ" else _lfq_mix_stress())
+
+
+def _lfq_mix_stress():
+    # the same run on G-LFQ (no slow path: the retry loops take its place)
+    q = make("G-LFQ", 64, max_threads=64, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
+    try:
+        for rep in range(6):
+            r = gq.run_split(q, threads=64, block_threads=32, ops_per_thread=40000, producer_fraction=0.5, seed=7 + rep, role_layout=1,
+                             value_base=rep * 64 * 40000)
+            conserve(r, gq.queue_drain(q, 129))
+    finally:
+        gq.queue_destroy(q)
+    return "conserved"
 
 
 @pytest.mark.parametrize("kind", ["YMC-p0", "YMC-p1"])
@@ -280,8 +308,12 @@ def test_ymc_slow_paths_are_exercised(kind):
     for seed in range(3, 11):
         q = make(kind, 256, max_threads=256, flags=gq.GQ_F_NO_DEQ_SPIN | gq.GQ_F_NO_PROBE)
         try:
-            r = gq.run_split(q, threads=256, block_threads=64, ops_per_thread=64, producer_fraction=0.5, seed=seed, jitter_ns=seed * 40)
-            left = gq.queue_drain(q, 1 << 15)
+            # odd seeds: roles placed on homogeneous warps, so that producers and consumers run side by side (the two role
+            # loops of a mixed warp are divergent paths, which the hardware may run one after the other)
+            # and fixed duration instead of fixed operation counts, so that the consumers are still polling when items arrive
+            r = gq.run_split(q, threads=256, block_threads=64, warmup_ms=0.0, duration_ms=2.0, producer_fraction=0.5, seed=seed,
+                             role_layout=seed & 1)
+            left = gq.queue_drain(q, 1 << 22)
         finally:
             gq.queue_destroy(q)
         assert r["pool_exhausted"] == 0
