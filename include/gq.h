@@ -146,6 +146,9 @@ typedef struct {
   uint32_t converged;          /* 1: the lanes of a warp start every iteration of the benchmark loop together (one ballot per
                                   iteration), as a lock-step wavefront would; 0: a lane starts its next operation as soon as its
                                   last one returns.  Balanced and split loops; not the fused role_layout 2 */
+  uint32_t block_faa;          /* 1: the warps of a block combine their ticket requests per hot counter in shared memory: one global
+                                  FAA per batch instead of one per warp (block-level funnel, D11; include/gq/queue.cuh) */
+  uint32_t funnel_window_ns;   /* block_faa: a batch stays open this long so that more warps can join (0 = closed at once) */
 } gq_run_cfg;
 
 typedef struct {
@@ -175,6 +178,12 @@ int run_slot_atomic_ceiling(const gq_run_cfg* cfg, uint64_t slots, gq_run_result
    seeded divergent control flow; tickets_out (HOST, threads*rounds entries, UINT64_MAX = lane did
    not participate that round); *final_counter = counter value at the end. */
 int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint64_t* tickets_out, uint64_t* final_counter);
+
+/* The same probe with the tickets drawn through a block-level funnel (D11; blocks of 256 threads, one funnel per
+   block): Lemma III.1 must hold batch-wise.  tickets_out may be NULL (long runs); sum_count_out (HOST, 2 words, may be NULL)
+   = sum of all tickets handed out and their number: with distinct tickets 0..m-1 the sum is m(m-1)/2. */
+int run_funnel_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint32_t funnel_window_ns, uint64_t* tickets_out,
+                     uint64_t* final_counter, uint64_t* sum_count_out);
 
 /* Single-thread script: op[i] in {GQ_OP_ENQ, GQ_OP_DEQ}, arg[i] payload; results to HOST arrays.
    `tid` = the thread_ctx id used (exercises per-thread records). */

@@ -12,6 +12,7 @@
 // 32-lane warps with independent thread scheduling (reading G10).
 #pragma once
 #include <cstdint>
+#include <cstdio>
 
 #include "debug.cuh"
 
@@ -89,6 +90,37 @@ __device__ __forceinline__ uint32_t cas_acq_rel32(uint32_t* p, uint32_t expected
   uint32_t o; asm volatile("atom.acq_rel.gpu.global.cas.b32 %0, [%1], %2, %3;" : "=r"(o) : "l"(p), "r"(expected), "r"(desired) : "memory"); return o;
 }
 
+// ---- block-level ticket funnel (D11; "Aggregating Funnels ... our G-LFQ uses this direction as
+//      inspiration", L95) ------------------------------------------------------------------------------------------
+// One BlockFunnel per (thread block, hot counter), in shared memory.  The leaders of the warps of a block that ask for
+// tickets of the same counter at about the same time are combined into ONE global FAA:
+//   join    : old = atomicAdd(gate, <1 warp, cnt tickets>)   ->  batch number, place in the batch, ticket offset
+//   combine : the warp that opened the batch (place 0) closes it with atomicExch(gate, <next batch, 0, 0>), issues
+//             FAA(counter, total) and publishes the base in the batch's slot;
+//   follow  : every other warp of the batch waits for that slot and takes base + its offset.
+// Nobody waits for a warp that is not already executing these very steps: a follower waits for its combiner, which is
+// inside its FAA; a combiner waits only for the previous tenant of its slot (an older batch, same argument).  A warp
+// that finds the gate idle pays two shared-memory atomics more than the plain WAVEFAA.  `window_ns` > 0 keeps a batch
+// open that long so that more warps can join (fewer global atomics against a longer wait for the ticket).
+// Lemma III.1 carries over batch-wise: one FAA of `total` hands out `total` distinct consecutive tickets, each warp gets
+// the contiguous sub-range [off, off + cnt), each lane its rank inside it.
+constexpr uint32_t kFunnelSlots = 8;
+struct FunnelSlot { unsigned long long base; unsigned int seq; unsigned int readers; };
+struct alignas(16) BlockFunnel {
+  unsigned long long gate;                  // [63:32] batch | [31:16] warps joined | [15:0] tickets asked
+  unsigned int window_ns, _pad;
+  FunnelSlot slot[kFunnelSlots];
+};
+// call with the whole block before first use (ends with __syncthreads)
+__device__ __forceinline__ void funnel_init(BlockFunnel* f, uint32_t n, uint32_t window_ns) {
+  for (uint32_t i = threadIdx.x; i < n * kFunnelSlots; i += blockDim.x) {
+    FunnelSlot* s = &f[i / kFunnelSlots].slot[i % kFunnelSlots];
+    s->base = 0; s->readers = 0; s->seq = (i % kFunnelSlots) - kFunnelSlots;      // "batch seq - slots was published and read"
+  }
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) { f[i].gate = 0; f[i].window_ns = window_ns; }
+  __syncthreads();
+}
+
 // ---- WAVEFAA --------------------------------------------------------------------------
 // PAPER.md Alg. 1: mask <- Ballot(active); count <- Popcount(mask); leader <-
 // FirstSetBit(mask)-1; leader: base <- FAA(C, count); base <- Shuffle(base, leader);
@@ -102,8 +134,51 @@ __device__ __forceinline__ uint32_t cas_acq_rel32(uint32_t* p, uint32_t expected
 // and no lane waits for a lane outside its own mask (reading G10).  `unit` scales the add
 // for packed counters (G-WFQ: unit = 1 << THRIDX_BITS); the returned value is the raw word
 // base + rank*unit.
+// The funnel steps of one WAVEFAA group (mask, leader), executed by ALL lanes of the group together: only single atomics sit
+// inside `if (lead)`, every wait is a loop the whole group runs converged, and results travel by __shfl_sync(mask).
+// (Measured on sm_100a: when only the leader waited, inside a divergent region, with its group parked at the compiler's
+//  reconvergence barrier, other diverged groups of the same warp passing through the same code released that barrier
+//  early and the group read the leader's base before it was there.  No lane may wait for another one at a BSYNC.)
+__device__ __forceinline__ uint64_t funnel_faa(BlockFunnel* f, uint64_t* counter, uint64_t unit, uint32_t mask, uint32_t leader) {
+  const bool lead = lane_id() == leader;
+  unsigned long long old = 0;
+  if (lead) old = atomicAdd(&f->gate, (1ull << 16) | (unsigned long long)__popc(mask));          // join
+  old = __shfl_sync(mask, old, leader);
+  const uint32_t seq = (uint32_t)(old >> 32), place = (uint32_t)(old >> 16) & 0xFFFFu, off = (uint32_t)old & 0xFFFFu;
+  FunnelSlot* s = &f->slot[seq & (kFunnelSlots - 1)];
+  volatile unsigned int* vseq = &s->seq;
+  volatile unsigned int* vreaders = &s->readers;
+  if (place != 0) {                                                   // follow (the whole group)
+    while (*vseq != seq) __nanosleep(20);                             // the nap lets diverged lanes of this very warp run: the combiner may be one
+    const uint64_t base = *reinterpret_cast<volatile unsigned long long*>(&s->base);
+    if (lead) atomicSub(&s->readers, 1u);
+    return base + (uint64_t)off * unit;
+  }
+  if (f->window_ns) __nanosleep(f->window_ns);                        // combine
+  unsigned long long closed = 0;
+  if (lead) closed = atomicExch(&f->gate, (unsigned long long)(seq + 1u) << 32);
+  closed = __shfl_sync(mask, closed, leader);
+  const uint32_t total = (uint32_t)closed & 0xFFFFu, warps = (uint32_t)(closed >> 16) & 0xFFFFu;
+  uint64_t base = 0;
+  if (lead) base = faa_relaxed(counter, (uint64_t)total * unit);
+  base = __shfl_sync(mask, base, leader);                             // the group waits for the FAA here, converged
+#ifdef GQ_DBG_SITES
+  if (lead && (blockIdx.x & 63u) == 0) { GQ_COUNT(22, 1); GQ_COUNT(23, warps); }   // funnel batches, groups per batch (sampled blocks)
+#endif
+  {
+    while (*vseq != seq - kFunnelSlots || *vreaders != 0) __nanosleep(20);   // previous tenant of the slot published and read
+    if (lead) {
+      *reinterpret_cast<volatile unsigned long long*>(&s->base) = base;
+      *vreaders = warps - 1u;
+      __threadfence_block();
+      *vseq = seq;
+    }
+  }
+  return base;
+}
+
 template <bool kUniform>
-__device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 1) {
+__device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 1, BlockFunnel* funnel = nullptr) {
   uint32_t mask = __activemask();
   if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
 #ifdef GQ_DBG_SITES
@@ -111,6 +186,7 @@ __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 
 #endif
   const uint32_t leader = __ffs(mask) - 1;
   const uint32_t rank = __popc(mask & lanemask_lt()) + (GQ_MUT(MUT_RANK_OFF_BY_ONE) ? 1u : 0u);
+  if (funnel) return funnel_faa(funnel, counter, unit, mask, leader) + (uint64_t)rank * unit;   // all lanes of one group name one funnel
   uint64_t base = 0;
   if (lane_id() == leader) {
     base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);

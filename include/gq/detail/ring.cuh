@@ -32,6 +32,8 @@ struct RingView {
   uint32_t  prefetch;   // > 0: rings too large to stay L2-resident: pull the slot `prefetch` tickets ahead into L2
   uint32_t  id;         // 0 = AQ (or the only ring), 1 = FQ: names the ring in traces and latency probes (debug.cuh)
   uint32_t  spin_ns;    // D2: a parked dequeuer re-reads its slot without any nap for this long, then backs off
+  detail::BlockFunnel* fhead;   // block-level ticket funnels of the calling block (shared memory; D11), or nullptr:
+  detail::BlockFunnel* ftail;   // set by the kernel on its own copy of the view (with_funnels, queue.cuh)
 };
 
 namespace detail {
@@ -166,7 +168,7 @@ struct NoFinalize {
 };
 
 
-template <class F, bool kUniform, bool kWarpFaa = true>
+template <class F, bool kUniform, int kWarpFaa = true>
 struct Ring {
   __device__ __forceinline__ static uint64_t* slot(const RingView& r, uint32_t j) {
     return r.entry + ((size_t)j << r.slot_shift);
@@ -175,10 +177,12 @@ struct Ring {
   __device__ __forceinline__ static uint32_t cycle_of(const RingView& r, uint64_t t) { return (uint32_t)(t >> r.order) & F::kCycMask; }
   __device__ __forceinline__ static uint64_t counter(uint64_t word) { return word >> F::kCtrShift; }
 
-  // ticket reservation: WAVEFAA on a (possibly packed) counter word
-  __device__ __forceinline__ static uint64_t take(uint64_t* ctr) {
+  // ticket reservation: WAVEFAA on a (possibly packed) counter word, through the block's funnel when it has one
+  __device__ __forceinline__ static uint64_t take(const RingView& r, bool head) {
     constexpr uint64_t unit = 1ull << F::kCtrShift;
-    const uint64_t w = kWarpFaa ? warp_faa<kUniform>(ctr, unit) : lane_faa(ctr, unit);
+    uint64_t* ctr = head ? r.head : r.tail;
+    // kWarpFaa: 0 = one FAA per thread (ablation), 1 = WAVEFAA, 2 = WAVEFAA through the block's funnels (D11)
+    const uint64_t w = kWarpFaa ? warp_faa<kUniform>(ctr, unit, kWarpFaa == 2 ? (head ? r.fhead : r.ftail) : nullptr) : lane_faa(ctr, unit);
     return counter(w);
   }
 
@@ -244,7 +248,7 @@ struct Ring {
   __device__ __forceinline__ static int try_enq(const RingView& r, uint32_t x, uint64_t* t_out, uint32_t flags = 0,
                                                 bool have = false, uint64_t t_pre = 0) {
     GQ_TIC(t0);
-    const uint64_t t = have ? t_pre : take(r.tail);                   // L144
+    const uint64_t t = have ? t_pre : take(r, false);                   // L144
     if (!have) GQ_TOC(LAT_TAIL_FAA + 5 * r.id, t0, t);
     *t_out = t;
     // A first-touch CAS is an L2 miss that the slice's atomic unit waits out, with every atomic queued behind
@@ -328,11 +332,11 @@ struct Ring {
         if (GQ_MUT(MUT_UNSOUND_EMPTY) && T <= H + 2) return RING_EMPTY;
         if (T + ((park_ns && !(flags & kEagerEmpty)) ? r.park_limit : 0u) <= H) { GQ_SITE(SITE_DEQ_EMPTY_PROBE); return RING_EMPTY; }
       }
-      h = take(r.head);                                               // L172
+      h = take(r, true);                                               // L172
       thr = r.thr_reset;                                              // parking allowed (as before D4)
     } else {
       thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));   // in flight with the FAA / slot load
-      h = take(r.head);                                               // L172
+      h = take(r, true);                                               // L172
     }
     GQ_TOC(LAT_HEAD_FAA + 5 * r.id, t0, h);
     *h_out = h;

@@ -21,7 +21,7 @@ struct DlfqView {
   uint32_t flags;     // GQ_F_*
 };
 
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const DlfqView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
@@ -36,7 +36,7 @@ __device__ __forceinline__ int enqueue(const DlfqView& q, thread_ctx& ctx, uint3
   return OK;
 }
 
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int dequeue(const DlfqView& q, thread_ctx& ctx, uint32_t* out, uint64_t* retries = nullptr) {
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;

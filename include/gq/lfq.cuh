@@ -32,7 +32,7 @@ struct LfqView {
 
 namespace detail {
 
-template <class F, bool kUniform, bool kWarpFaa, class Fin>
+template <class F, bool kUniform, int kWarpFaa, class Fin>
 __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, uint64_t* retries, const Fin& fin,
                                              bool probe, uint32_t flags, uint64_t* ticket = nullptr) {
   Backoff bo;
@@ -47,7 +47,7 @@ __device__ __forceinline__ int ring_deq_loop(const RingView& r, uint32_t* idx, u
     bo.pause();
   }
 }
-template <class F, bool kUniform, bool kWarpFaa>
+template <class F, bool kUniform, int kWarpFaa>
 __device__ __forceinline__ void ring_enq_loop(const RingView& r, uint32_t idx, uint64_t* retries, uint32_t flags) {
   Backoff bo;
   [[maybe_unused]] uint32_t sn = 0;
@@ -98,7 +98,7 @@ __device__ __forceinline__ uint64_t cell_await(const uint64_t* cell, uint64_t w,
 }  // namespace detail
 
 // kUniform: all lanes converged at the call name the same queue (see warp_faa).
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
   using R = Ring<LfqFmt, kUniform, kWarpFaa>;
@@ -121,7 +121,7 @@ __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32
   for (;;) {
     if (GQ_STUCK(sn, 3, ctx.tid, q.aq.head, q.aq.tail)) return OK;
     GQ_TIC(t0);
-    const uint64_t t = R::take(q.aq.tail);
+    const uint64_t t = R::take(q.aq, false);
     GQ_TOC(LAT_TAIL_FAA, t0, t);
     if (!GQ_MUT(MUT_NO_HANDSHAKE)) st_relaxed(cell, cell_word(t, v));   // D6: payload tagged with its ticket
     uint64_t tt;
@@ -137,7 +137,7 @@ __device__ __forceinline__ int enqueue(const LfqView& q, thread_ctx& ctx, uint32
 // FQ tail ticket is reserved while the payload load is still in flight: the two L2 round trips
 // overlap.  No speculation (the ticket is always used at once) and no waiting on another thread
 // while it is held.  GQ_F_NO_PAIRED_FAA restores load-then-reserve.
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32_t* out, uint64_t* retries = nullptr) {
   using namespace detail;
   using R = Ring<LfqFmt, kUniform, kWarpFaa>;
@@ -157,7 +157,7 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
   uint64_t w = ld_relaxed(cell);                                   // after the acquire load of the entry
   const bool paired = !(q.flags & kNoPairedFaa) && !GQ_MUT(MUT_EARLY_RECYCLE);
   uint64_t t = 0;
-  if (paired) t = R::take(q.fq.tail);                              // D5: issued behind the payload load
+  if (paired) t = R::take(q.fq, false);                              // D5: issued behind the payload load
   if (!fenced) w = cell_await(cell, w, ctx.last_ticket);
   GQ_TOC(LAT_PAYLOAD, t0, w + t);
   *out = (uint32_t)w;
@@ -183,7 +183,7 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
 // two roles overlap.  *v is the payload (in) for is_enq lanes and the result (out) for the others.
 // Returns OK, FULL (enqueue lanes) or EMPTY (dequeue lanes).  Ticket-tagged cells (D6) only; with
 // GQ_F_FENCED_PAYLOAD it falls back to the two separate calls.
-template <bool kWarpFaa = true>
+template <int kWarpFaa = true>
 __device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& ctx, bool is_enq, uint32_t* v, uint64_t* retries = nullptr) {
   using namespace detail;
   using R = Ring<LfqFmt, false, kWarpFaa>;
@@ -205,7 +205,7 @@ __device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& 
   [[maybe_unused]] uint32_t sn = 0;
   for (bool first = true;; first = false) {
     if (GQ_STUCK(sn, 4, ctx.tid, r2.head, r2.tail)) return OK;
-    const uint64_t t = R::take(r2.tail);                               // two leaders, one instruction
+    const uint64_t t = R::take(r2, false);                               // two leaders, one instruction
     if (is_enq) {
       st_relaxed(cell, cell_word(t, *v));                              // D6: payload tagged with its AQ ticket
     } else if (first) {

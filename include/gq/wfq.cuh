@@ -279,7 +279,7 @@ struct Wf {
   // have_pre/t_pre: a tail ticket the caller reserved already (D5), used by the first fast attempt.
   // cell/v (AQ side with D6): every fast attempt stores <its ticket | v> into the payload cell and
   // installs x | kWfqFast with a relaxed CAS; the slow path installs plain x behind the record's fences.
-  template <bool kUniform, bool kWarpFaa>
+  template <bool kUniform, int kWarpFaa>
   __device__ static void ring_enq(const RingView& r, uint32_t x, uint32_t patience, uint32_t me, uint64_t* retries, uint32_t flags,
                                   bool have_pre = false, uint64_t t_pre = 0, uint64_t* cell = nullptr, uint32_t v = 0) {
     using R = Ring<F, kUniform, kWarpFaa>;
@@ -292,7 +292,7 @@ struct Wf {
     }
     for (uint32_t p = have_pre ? 1 : 0; p < patience; ++p) {
       if (cell) {
-        const uint64_t tk = R::take(r.tail);
+        const uint64_t tk = R::take(r, false);
         st_relaxed(cell, cell_word(tk, v));
         if (R::try_enq(r, x | kWfqFast, &t, flags | kRelaxedInstall, true, tk) == RING_OK) return;
       } else if (R::try_enq(r, x, &t, flags) == RING_OK) return;
@@ -327,7 +327,7 @@ struct Wf {
     st_release(&my->seq1, s + 1);
   }
 
-  template <bool kUniform, bool kWarpFaa>
+  template <bool kUniform, int kWarpFaa>
   __device__ static int ring_deq(const RingView& r, uint32_t* x, uint32_t patience, uint32_t me, uint32_t nthreads,
                                  uint64_t* retries, bool probe, uint32_t flags, uint64_t* ticket = nullptr) {
     const Finalize fin{nthreads};
@@ -396,7 +396,7 @@ __device__ __forceinline__ void wfq_help_threads(const WfqView& q, thread_ctx& c
 
 }  // namespace detail
 
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
@@ -418,7 +418,7 @@ __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32
   return OK;
 }
 
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32_t* out, uint64_t* retries = nullptr) {
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
@@ -438,7 +438,7 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   // delivered its value (control dependency), so the fast-path install needs no release fence.
   const bool paired = !(q.flags & kNoPairedFaa) && q.enq_patience != 0 && q.enq_patience != 0xFFFFFFFFu;
   uint64_t t = 0;
-  if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq.tail);
+  if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq, false);
   if (fast) w = cell_await(cell, w, ctx.last_ticket);               // tagged cell: wait for the store of THIS tenure of idx
   *out = (uint32_t)w;
   GQ_IDX_EVENT(7, q.aq, idx, ctx.last_ticket, w, fast);

@@ -56,6 +56,8 @@ struct YmcView {
   uint32_t enq_patience, deq_patience, help_delay;
   uint32_t flags;
   uint32_t park_ns, park_limit, park_nap, _pad;
+  detail::BlockFunnel* fhead;   // block-level ticket funnels of the calling block (D11), or nullptr
+  detail::BlockFunnel* ftail;
 };
 
 namespace detail {
@@ -74,9 +76,9 @@ struct Ymc {
   }
   __device__ __forceinline__ static uint32_t next(const YmcView& q, uint32_t p) { return p + 1 < q.nthreads ? p + 1 : 0; }
 
-  template <bool kUniform, bool kWarpFaa>
-  __device__ __forceinline__ static uint64_t take(uint64_t* ctr) {
-    return kWarpFaa ? warp_faa<kUniform>(ctr) : lane_faa(ctr);
+  template <bool kUniform, int kWarpFaa>
+  __device__ __forceinline__ static uint64_t take(uint64_t* ctr, BlockFunnel* f = nullptr) {
+    return kWarpFaa ? warp_faa<kUniform>(ctr, 1, kWarpFaa == 2 ? f : nullptr) : lane_faa(ctr);
   }
   // [5] advance_end_for_linearizability: E <- max(E, cid), one native atom.max
   __device__ __forceinline__ static void advance(uint64_t* E, uint64_t cid) {
@@ -175,7 +177,7 @@ struct Ymc {
 
 }  // namespace detail
 
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
   using Y = Ymc;
@@ -183,7 +185,7 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
   uint64_t id = 0;
   // fast path ([5] enq_fast): ticket, then one CAS bot -> value
   for (uint32_t p = 0; p < q.enq_patience; ++p) {
-    const uint64_t i = Y::take<kUniform, kWarpFaa>(q.tail);
+    const uint64_t i = Y::take<kUniform, kWarpFaa>(q.tail, q.ftail);
     if (i >= Y::last(q)) { Y::pool_exhausted(q); return FULL; }
     // Cells are never reused, so every deposit CAS would be the first touch of its line: an L2 miss
     // that the atomic unit of that slice waits out, and with it every other atomic queued there, the FAAs on
@@ -234,7 +236,7 @@ __device__ __forceinline__ int enqueue(const YmcView& q, thread_ctx& ctx, uint32
   return OK;
 }
 
-template <bool kUniform = false, bool kWarpFaa = true>
+template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int dequeue(const YmcView& q, thread_ctx& ctx, uint32_t* out, uint64_t* retries = nullptr) {
   using namespace detail;
   using Y = Ymc;
@@ -255,7 +257,7 @@ __device__ __forceinline__ int dequeue(const YmcView& q, thread_ctx& ctx, uint32
       const uint64_t T = ld_relaxed(q.tail);                  // caught up over burnt cells, reading Y9), which says
       if (T <= H) { w = Y::kEmptyRet; break; }                // nothing about cells ahead; Tail <= Head does
     }
-    const uint64_t i = Y::take<kUniform, kWarpFaa>(q.head);
+    const uint64_t i = Y::take<kUniform, kWarpFaa>(q.head, q.fhead);
     w = Y::help_enq(q, ctx.tid, i, park_ns);
     if (w == Y::kEmptyRet) {                                  // T <= i was observed: the queue is empty
       // Catch T up to i + 1 (reading Y9; the ring's L200 "catch up Tail" carried over).  Without it every

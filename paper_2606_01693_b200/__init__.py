@@ -27,9 +27,15 @@ KIND_NAMES = {GQ_LFQ: "G-LFQ", GQ_WFQ: "G-WFQ", GQ_WFQ_YMC: "G-WFQ-YMC", GQ_LFQ_
 _ERR = {-1: "INVAL", -2: "NOMEM", -3: "CUDA", -4: "RESIDENCY", -5: "TIMEOUT", -6: "STATE", -7: "POOL"}
 
 
+TIMED_OUT = False      # set once a call returned GQ_E_TIMEOUT: the kernel is still running, every later CUDA call would block on it
+
+
 class GqError(RuntimeError):
     def __init__(self, code, where):
+        global TIMED_OUT
         self.code = code
+        if code == GQ_E_TIMEOUT:
+            TIMED_OUT = True
         detail = lib.gq_last_cuda_error().decode() if code in (GQ_E_CUDA, GQ_E_TIMEOUT, GQ_E_NOMEM) else ""
         super().__init__(f"{where}: GQ_E_{_ERR.get(code, code)} {detail}".strip())
 
@@ -46,7 +52,7 @@ class gq_run_cfg(C.Structure):
                 ("duration_ms", C.c_double), ("producer_fraction", C.c_double), ("seed", C.c_uint64),
                 ("record_history", C.c_uint32), ("ops_per_thread", C.c_uint32), ("jitter_ns", C.c_uint32),
                 ("fail_backoff_ns", C.c_uint32), ("value_base", C.c_uint64),
-                ("role_layout", C.c_uint32), ("converged", C.c_uint32)]
+                ("role_layout", C.c_uint32), ("converged", C.c_uint32), ("block_faa", C.c_uint32), ("funnel_window_ns", C.c_uint32)]
 
 
 class gq_run_result(C.Structure):
@@ -86,7 +92,7 @@ HIST_DTYPE = np.dtype([("proc", "<u4"), ("op", "<u4"), ("arg", "<u4"), ("ret_sta
 # every symbol include/gq.h declares
 SYMBOLS = ("queue_storage_bytes", "queue_create", "queue_create_ex", "queue_destroy", "queue_reset", "queue_prefill",
            "queue_drain", "queue_device_view", "queue_kind", "queue_max_coresident_threads", "run_balanced",
-           "run_split", "run_faa_ceiling", "run_slot_atomic_ceiling", "run_warp_faa_probe", "queue_run_script",
+           "run_split", "run_faa_ceiling", "run_slot_atomic_ceiling", "run_warp_faa_probe", "run_funnel_probe", "queue_run_script",
            "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "gq_last_cuda_error", "gq_version",
            "gq_dbg_sites", "gq_dbg_trace", "gq_set_mutation", "queue_debug_counters")
 
@@ -112,6 +118,7 @@ def _load(variant=""):
     L.run_faa_ceiling.argtypes = [P(gq_run_cfg), C.c_uint32, P(gq_run_result)]
     L.run_slot_atomic_ceiling.argtypes = [P(gq_run_cfg), C.c_uint64, P(gq_run_result)]
     L.run_warp_faa_probe.argtypes = [C.c_uint32, C.c_uint32, C.c_uint64, C.c_void_p, P(C.c_uint64)]
+    L.run_funnel_probe.argtypes = [C.c_uint32, C.c_uint32, C.c_uint64, C.c_uint32, C.c_void_p, P(C.c_uint64), C.c_void_p]
     L.queue_run_script.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
     L.history_dump.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(C.c_uint64)]
     L.bfs_run.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, P(gq_bfs_stats), C.c_void_p]
@@ -259,6 +266,15 @@ def run_warp_faa_probe(threads, rounds, seed):
     fin = C.c_uint64(0)
     _chk(lib.run_warp_faa_probe(threads, rounds, seed, _np_ptr(t), C.byref(fin)), "run_warp_faa_probe")
     return t.reshape(threads, rounds), fin.value
+
+
+def run_funnel_probe(threads, rounds, seed, window_ns=0, keep_tickets=True):
+    """(tickets or None, final counter, sum of tickets, number of tickets)"""
+    t = np.empty(threads * rounds, np.uint64) if keep_tickets else None
+    fin = C.c_uint64(0)
+    sc = np.zeros(2, np.uint64)
+    _chk(lib.run_funnel_probe(threads, rounds, seed, window_ns, _np_ptr(t) if keep_tickets else None, C.byref(fin), _np_ptr(sc)), "run_funnel_probe")
+    return (t.reshape(threads, rounds) if keep_tickets else None), fin.value, int(sc[0]), int(sc[1])
 
 
 def queue_run_script(q, ops, args, tid=0):

@@ -31,7 +31,7 @@ static int cuda_fail(cudaError_t e, const char* what) { return gq_cuda_fail(e, w
 extern "C" const char* gq_last_cuda_error(void) { return g_err; }
 extern "C" const char* gq_version(void) { return "gq 0.1 (sm_100a)"; }
 
-static_assert(sizeof(gq_opts) == 64 && sizeof(gq_run_cfg) == 72 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
+static_assert(sizeof(gq_opts) == 64 && sizeof(gq_run_cfg) == 80 && sizeof(gq_run_result) == 144 && sizeof(gq_hist_rec) == 40,
               "ABI structs: the Python binding mirrors these layouts");
 
 // ------------------------------------------------------------------------------- handle
@@ -259,7 +259,7 @@ static int format_queue(gq_queue* q, cudaStream_t st) {
 template <class Q>
 static int max_blocks_per_sm(int block_threads) {
   int nb = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, bench_kernel<Q, false, true>, block_threads, 0) != cudaSuccess) return 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, bench_kernel<Q, false, 1>, block_threads, 0) != cudaSuccess) return 0;
   return nb;
 }
 static int kind_blocks_per_sm(int kind, int block_threads) {
@@ -552,6 +552,7 @@ static BenchParams make_params(const gq_run_cfg* cfg, const Resolved& r, int mod
   p.seed = (uint32_t)cfg->seed; p.ops_per_thread = cfg->ops_per_thread;
   p.jitter_ns = cfg->jitter_ns; p.fail_backoff_ns = cfg->fail_backoff_ns; p.value_base = cfg->value_base;
   p.converged = cfg->converged;
+  p.block_faa = cfg->block_faa; p.funnel_window_ns = cfg->funnel_window_ns;
   // history runs small enough for it use the payload encoding of BASELINE.json configs[0]: thread << 16 | iteration
   p.tid_shift = (cfg->record_history && r.threads <= 65536 && cfg->ops_per_thread <= 65536) ? 16u : 0u;
   return p;
@@ -631,9 +632,12 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   const bool fused = mode == MODE_SPLIT && cfg->role_layout == 2;       // mixed warps, one converged call (G-LFQ)
   if (fused && (q->kind != GQ_LFQ || per_lane)) return GQ_E_INVAL;
   if (hist && per_lane) return GQ_E_INVAL;                              // the per-thread-FAA ablation is a timing variant only
-  void* fn = hist ? (void*)bench_kernel<Q, true, true> : (per_lane ? (void*)bench_kernel<Q, false, false> : (void*)bench_kernel<Q, false, true>);
+  const bool funnel = cfg->block_faa != 0;                              // block-level ticket funnels (D11): a kernel variant of its own
+  if (funnel && (per_lane || fused)) return GQ_E_INVAL;
+  void* fn = hist ? (void*)bench_kernel<Q, true, 1> : (per_lane ? (void*)bench_kernel<Q, false, 0> : (void*)bench_kernel<Q, false, 1>);
+  if (funnel) fn = hist ? (void*)bench_kernel<Q, true, 2> : (void*)bench_kernel<Q, false, 2>;
   if constexpr (HasFused<Q>::value) {
-    if (fused) fn = hist ? (void*)bench_kernel<Q, true, true, true> : (void*)bench_kernel<Q, false, true, true>;
+    if (fused) fn = hist ? (void*)bench_kernel<Q, true, 1, true> : (void*)bench_kernel<Q, false, 1, true>;
   }
   Resolved r;
   int nb = 0;
@@ -752,21 +756,44 @@ extern "C" int run_slot_atomic_ceiling(const gq_run_cfg* cfg, uint64_t slots, gq
   return rc;
 }
 
-extern "C" int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint64_t* tickets_out, uint64_t* final_counter) {
-  if (!threads || !rounds || !tickets_out || !final_counter) return GQ_E_INVAL;
+static int faa_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint32_t funnel_mode, uint32_t window_ns,
+                     uint64_t* tickets_out, uint64_t* final_counter, uint64_t* sum_out) {
+  if (!threads || !rounds || !final_counter) return GQ_E_INVAL;
   if (device_sms() <= 0) { std::snprintf(g_err, sizeof g_err, "no CUDA device"); return GQ_E_CUDA; }
   uint64_t *d_c = nullptr, *d_t = nullptr;
   const size_t n = (size_t)threads * rounds;
-  CU(cudaMalloc(&d_c, 8));
-  cudaError_t e = cudaMalloc(&d_t, n * 8);
+  CU(cudaMalloc(&d_c, 32));
+  cudaError_t e = tickets_out ? cudaMalloc(&d_t, n * 8) : cudaSuccess;
   if (e != cudaSuccess) { cudaFree(d_c); return cuda_fail(e, "cudaMalloc"); }
-  cudaMemset(d_c, 0, 8);
-  warp_faa_probe_kernel<<<(threads + 255) / 256, 256>>>(d_c, threads, rounds, (uint32_t)seed, d_t);
-  e = cudaDeviceSynchronize();
-  if (e == cudaSuccess) e = cudaMemcpy(tickets_out, d_t, n * 8, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemcpy(final_counter, d_c, 8, cudaMemcpyDeviceToHost);
-  cudaFree(d_c); cudaFree(d_t);
-  return e == cudaSuccess ? 0 : cuda_fail(e, "warp_faa_probe");
+  cudaMemset(d_c, 0, 32);
+  LaunchRes lr;
+  int rc = lr.create();
+  if (rc == 0) {
+    warp_faa_probe_kernel<<<(threads + 255) / 256, 256>>>(d_c, threads, rounds, (uint32_t)seed, d_t, funnel_mode, window_ns,
+                                                          reinterpret_cast<unsigned long long*>(d_c + 1));
+    cudaEventRecord(lr.e1, nullptr);
+    rc = wait_event(lr.e1, watchdog_slack_s());
+  }
+  if (rc == GQ_E_TIMEOUT) { lr.abandon(); return rc; }
+  uint64_t h[3] = {0, 0, 0};
+  if (rc == 0) {
+    e = cudaMemcpy(h, d_c, 24, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && tickets_out) e = cudaMemcpy(tickets_out, d_t, n * 8, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) rc = cuda_fail(e, "warp_faa_probe");
+  }
+  cudaFree(d_c); if (d_t) cudaFree(d_t);
+  if (rc) return rc;
+  *final_counter = h[0];
+  if (sum_out) { sum_out[0] = h[1]; sum_out[1] = h[2]; }
+  return 0;
+}
+extern "C" int run_warp_faa_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint64_t* tickets_out, uint64_t* final_counter) {
+  if (!tickets_out) return GQ_E_INVAL;
+  return faa_probe(threads, rounds, seed, 0, 0, tickets_out, final_counter, nullptr);
+}
+extern "C" int run_funnel_probe(uint32_t threads, uint32_t rounds, uint64_t seed, uint32_t funnel_window_ns, uint64_t* tickets_out,
+                                uint64_t* final_counter, uint64_t* sum_count_out) {
+  return faa_probe(threads, rounds, seed, 1, funnel_window_ns, tickets_out, final_counter, sum_count_out);
 }
 
 // ------------------------------------------------------------------------------- prefill / drain / script / history

@@ -29,14 +29,15 @@ struct BenchParams {
   uint32_t tid_shift;          // > 0: payload = value_base + (thread << tid_shift | iter) (BASELINE.json configs[0]); 0: value_base + thread + iter * threads
   uint32_t _pad;
   uint32_t fused, converged;   // role_layout 2: mixed warps call the fused enqueue_or_dequeue (G-LFQ); converged: see gq_run_cfg
+  uint32_t block_faa, funnel_window_ns;   // block-level ticket funnels (gq_run_cfg)
 };
 
 // the fused mixed-warp operation exists for G-LFQ (lfq.cuh); other kinds run the two calls
 template <class Q> struct HasFused { static constexpr bool value = false; };
 template <> struct HasFused<LfqView> { static constexpr bool value = true; };
-template <bool kWarpFaa, class Q>
+template <int kWarpFaa, class Q>
 __device__ __forceinline__ int fused_op(const Q&, thread_ctx&, bool, uint32_t*, uint64_t*) { return -1; }
-template <bool kWarpFaa>
+template <int kWarpFaa>
 __device__ __forceinline__ int fused_op(const LfqView& q, thread_ctx& ctx, bool is_enq, uint32_t* v, uint64_t* retries) {
   return enqueue_or_dequeue<kWarpFaa>(q, ctx, is_enq, v, retries);
 }
@@ -62,7 +63,7 @@ __device__ __forceinline__ void fail_backoff(const BenchParams& p, Tally& a) {
   if (p.fail_backoff_ns) { a.fail_ns = a.fail_ns ? min(a.fail_ns * 2, p.fail_backoff_ns) : 64; __nanosleep(a.fail_ns); }
 }
 // one enqueue / one dequeue of the benchmark loop, with its history record (kHist) and its tallies; returns the end stamp
-template <class Q, bool kHist, bool kWarpFaa>
+template <class Q, bool kHist, int kWarpFaa>
 __device__ __forceinline__ uint64_t enq_step(const Q& q, thread_ctx& ctx, const BenchParams& p, uint32_t ltid, uint32_t iter,
                                              uint64_t tw, uint64_t te, Tally& a, gq_hist_rec*& my) {
   const uint32_t v = payload_of(p, ltid, iter);
@@ -80,7 +81,7 @@ __device__ __forceinline__ uint64_t enq_step(const Q& q, thread_ctx& ctx, const 
   else { ++a.tot_full; a.full += in; fail_backoff(p, a); }
   return now;
 }
-template <class Q, bool kHist, bool kWarpFaa>
+template <class Q, bool kHist, int kWarpFaa>
 __device__ __forceinline__ uint64_t deq_step(const Q& q, thread_ctx& ctx, const BenchParams& p, uint32_t ltid, uint32_t iter,
                                              uint64_t tw, uint64_t te, Tally& a, gq_hist_rec*& my) {
   uint32_t v = 0;
@@ -116,9 +117,14 @@ __device__ __forceinline__ bool loop_done(const BenchParams& p, uint32_t& act, b
 // producers and consumers run two separate loops.  One shared loop with `if (producer) ... if (consumer) ...` inside
 // makes the two halves of a mixed warp wait for each other at the reconvergence point of every iteration, i.e. run
 // one after the other (measured: 27 Gops/s at p = 0.5 against 56 with homogeneous warps).
-template <class Q, bool kHist, bool kWarpFaa, bool kFused = false>
+template <class Q, bool kHist, int kWarpFaa, bool kFused = false>
 __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint64_t* ctr, gq_hist_rec* hist) {
   cg::grid_group grid = cg::this_grid();
+  __shared__ BlockFunnel s_funnels[kWarpFaa == 2 ? kFunnelsPerQueue : 1];
+  if (kWarpFaa == 2) {                                  // D11: this block's ticket funnels, one per hot counter
+    funnel_init(s_funnels, kFunnelsPerQueue, p.funnel_window_ns);
+    q = with_funnels(q, s_funnels);
+  }
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
   if (tid == 0) st_relaxed(ctr + C_T0, globaltimer_ns());
   grid.sync();                                        // one time base for every thread
@@ -262,27 +268,36 @@ __global__ void script_kernel(Q q, const uint32_t* op, const uint32_t* arg, uint
 }
 
 // Lemma III.1 probe: warp_faa inside seeded, nested divergent control flow.
-__global__ void warp_faa_probe_kernel(uint64_t* counter, uint32_t threads, uint32_t rounds, uint32_t seed, uint64_t* tickets) {
+// funnel_mode: 0 = plain WAVEFAA, 1 = through a block-level funnel (D11) with window funnel_window_ns.  tickets == nullptr:
+// the tickets are only summed (long soak runs); *checksum then holds the sum of all tickets handed out.
+__global__ void warp_faa_probe_kernel(uint64_t* counter, uint32_t threads, uint32_t rounds, uint32_t seed, uint64_t* tickets,
+                                      uint32_t funnel_mode, uint32_t funnel_window_ns, unsigned long long* checksum) {
+  __shared__ BlockFunnel s_funnel[1];
+  if (funnel_mode) funnel_init(s_funnel, 1, funnel_window_ns);
+  BlockFunnel* f = funnel_mode ? s_funnel : nullptr;
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
   if (tid >= threads) return;
+  unsigned long long sum = 0, n = 0;
   for (uint32_t r = 0; r < rounds; ++r) {
     const uint32_t h = mix32(seed ^ (tid * 0x9e3779b9u) ^ (r * 0x85ebca6bu));
     uint64_t t = ~0ull;
     if (h & 1) {                       // participate?
       if (h & 2) {                     // two diverged groups name the same counter
         if (h & 4) __nanosleep(h >> 24);
-        t = warp_faa<true>(counter);
+        t = warp_faa<true>(counter, 1, f);
       } else {
-        t = warp_faa<false>(counter);  // address-matched variant
+        t = warp_faa<false>(counter, 1, f);  // address-matched variant
       }
+      sum += t; ++n;
     }
-    tickets[(size_t)tid * rounds + r] = t;
+    if (tickets) tickets[(size_t)tid * rounds + r] = t;
   }
+  if (checksum) { atomicAdd(checksum, sum); atomicAdd(checksum + 1, n); }
 }
 
 // Ceiling C1: bare WAVEFAA loop (BASELINE.json north_star: "a bare warp-aggregated FAA loop on one
 // counter at the same occupancy").  counters are 1 KiB apart.
-template <bool kWarpFaa>
+template <int kWarpFaa>
 __global__ void __launch_bounds__(512) faa_ceiling_kernel(uint64_t* counters, uint32_t n_counters, BenchParams p, uint64_t* ctr) {
   cg::grid_group grid = cg::this_grid();
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;

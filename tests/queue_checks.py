@@ -92,6 +92,16 @@ def check_warp_faa(threads, rounds, seed):
     return f"{len(took)} tickets"
 
 
+def check_funnel_faa(threads, rounds, seed, window_ns=0):
+    """Lemma III.1 through the block-level funnel (D11): distinct, contiguous tickets under seeded nested divergence."""
+    t, final, s, n = gq.run_funnel_probe(threads, rounds, seed, window_ns)
+    took = t[t != np.uint64(0xFFFFFFFFFFFFFFFF)]
+    assert final == len(took) == n, "counter != tickets handed out"
+    assert np.array_equal(np.sort(took), np.arange(len(took), dtype=np.uint64)), "funnel tickets not distinct and contiguous"
+    assert s == n * (n - 1) // 2
+    return f"{len(took)} tickets"
+
+
 # ---------------------------------------------------------------- single thread == sequential model
 def check_single_thread(kind, capacity, n_ops=6000):
     rng = np.random.default_rng(capacity)
@@ -126,11 +136,11 @@ def check_prefill_drain(kind, capacity, count):
 
 
 # ---------------------------------------------------------------- BJ config 1: tiny history
-def check_tiny_balanced(kind, seed, **opts):
+def check_tiny_balanced(kind, seed, run_kw=None, **opts):
     q = make(kind, 128, max_threads=64, park_ns=8000, **opts)
     try:
         r = gq.run_balanced(q, threads=64, block_threads=64, ops_per_thread=16, record_history=1,
-                            jitter_ns=200, seed=seed)
+                            jitter_ns=200, seed=seed, **(run_kw or {}))
         recs = gq.history_dump(q)
         left = gq.queue_drain(q, 256)
     finally:
@@ -203,7 +213,7 @@ def check_token_protocol(kind, threads=16384, ops=24):
 
 
 # ---------------------------------------------------------------- linearizability beyond the tiny config
-def check_medium_history(kind, threads, ops, capacity, max_fail_returns=4096):
+def check_medium_history(kind, threads, ops, capacity, max_fail_returns=4096, run_kw=None):
     """65 536 recorded operations from 4096 threads (128 warps over several SMs), k <= n and k > n (index starvation:
     dequeuers of FQ park, D2).  Too large for the exact WGL search at this overlap, but for histories whose returns are
     all OK / EMPTY with unique values the bad-pattern characterisation (oracle.poly) is exact, so OK here IS a
@@ -212,7 +222,7 @@ def check_medium_history(kind, threads, ops, capacity, max_fail_returns=4096):
     a run with more than max_fail_returns of them FAILS (parking, D2, is there to absorb the starvation)."""
     q = make(kind, capacity, max_threads=threads, **(dict(ymc_pool_cells=1 << 24) if is_ymc(kind) else {}))
     try:
-        r = gq.run_balanced(q, threads=threads, ops_per_thread=ops, record_history=1, jitter_ns=100, seed=11)
+        r = gq.run_balanced(q, threads=threads, ops_per_thread=ops, record_history=1, jitter_ns=100, seed=11, **(run_kw or {}))
         recs = gq.history_dump(q)
         left = gq.queue_drain(q, capacity + threads + 1)
     finally:

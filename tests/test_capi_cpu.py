@@ -29,7 +29,7 @@ def test_header_symbols_are_exported():
 def test_struct_sizes_match_header():
     # sizes implied by the field lists in gq.h (natural alignment)
     assert ctypes.sizeof(gq.gq_opts) == 64
-    assert ctypes.sizeof(gq.gq_run_cfg) == 72
+    assert ctypes.sizeof(gq.gq_run_cfg) == 80
     assert ctypes.sizeof(gq.gq_run_result) == 14 * 8 + 16 + 16
     assert gq.HIST_DTYPE.itemsize == 40
 

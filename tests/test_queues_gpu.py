@@ -15,7 +15,8 @@ import pytest
 import oracle
 import paper_2606_01693_b200 as gq
 from queue_checks import (VARIANTS, check_balanced_fixed_ops, check_medium_history, check_prefill_drain, check_single_thread,
-                          check_tiny_balanced, check_tiny_split, check_token_protocol, check_warp_faa, check_slow_fast_mix_stress, conserve, is_direct,
+                          check_tiny_balanced, check_tiny_split, check_token_protocol, check_warp_faa, check_funnel_faa, check_slow_fast_mix_stress, conserve,
+                          is_direct,
                           is_ymc, make, model_capacity, soft_slack, to_history, history_verdict, WGL_TALLY)
 
 pytestmark = pytest.mark.gpu
@@ -30,6 +31,17 @@ IDS = KINDS
 @pytest.mark.parametrize("threads,rounds,seed", [(32, 8, 1), (5000, 64, 2), (65536 + 17, 16, 3)])
 def test_warp_faa_tickets_distinct_and_contiguous(threads, rounds, seed):
     check_warp_faa(threads, rounds, seed)
+
+
+@pytest.mark.parametrize("threads,rounds,seed,window", [(256, 64, 1, 0), (5000, 200, 2, 0), (65536 + 17, 40, 3, 0), (5000, 100, 4, 300)])
+def test_funnel_tickets_distinct_and_contiguous(threads, rounds, seed, window):
+    # the probe that found the reconvergence-barrier problem (D11): thousands of diverged groups per warp and block
+    check_funnel_faa(threads, rounds, seed, window)
+
+
+def test_funnel_tickets_long_run():
+    _, final, s, n = gq.run_funnel_probe(151552, 2000, 7, 0, keep_tickets=False)
+    assert final == n and s == (n * (n - 1) // 2) % 2**64
 
 
 # ---------------------------------------------------------------- single thread == sequential model
@@ -372,6 +384,33 @@ def test_soak_past_the_ticket_tag_wrap(kind):
                          [(k, 4096, 8, 512) for k in ["G-LFQ", "G-WFQ", "G-WFQ-YMC", "G-LFQ-listed"]])
 def test_medium_history_bad_pattern_check(kind, threads, ops, capacity):
     check_medium_history(kind, threads, ops, capacity, max_fail_returns=256)
+
+
+# ---------------------------------------------------------------- block-level ticket funnels (D11)
+@pytest.mark.parametrize("kind", BIG)
+@pytest.mark.parametrize("window", [0, 300])
+def test_block_funnel_histories_and_conservation(kind, window):
+    kw = dict(block_faa=1, funnel_window_ns=window)
+    for seed in (1, 2, 3):
+        check_tiny_balanced(kind, seed, run_kw=kw)                     # 2 warps of one block share the four funnels
+    check_medium_history(kind, 4096, 8, 8192, max_fail_returns=256, run_kw=kw)
+    if not is_direct(kind):
+        check_medium_history(kind, 4096, 8, 512, max_fail_returns=256, run_kw=kw)
+    # BJ config 2 / 3 shapes at full co-residency, shortened windows
+    q = make(kind, 1 << 16, **(dict(ymc_pool_cells=1 << 31) if is_ymc(kind) else {}))
+    try:
+        r = gq.run_balanced(q, threads=0, warmup_ms=5, duration_ms=20, converged=1, **kw)
+        left = gq.queue_drain(q, (1 << 19) if is_ymc(kind) else (1 << 16) + 1 + soft_slack(kind, 1 << 18))
+        conserve(r, left)
+        assert r["succ_enq"] > 0 and r["pool_exhausted"] == 0
+        gq.queue_reset(q)
+        pre = np.arange(1 << 15, dtype=np.uint32)
+        gq.queue_prefill(q, pre)
+        r = gq.run_split(q, threads=0, ops_per_thread=40, producer_fraction=0.5, seed=1, value_base=1 << 15, **kw)
+        left = gq.queue_drain(q, 1 << 23)
+        conserve(r, left, pre)
+    finally:
+        gq.queue_destroy(q)
 
 
 # ---------------------------------------------------------------- split with compacted roles
