@@ -226,6 +226,15 @@ typedef struct { uint32_t width, height, spp, max_bounce, n_spheres, threads; ui
                  const float* d_spheres; /* DEVICE, n_spheres x 8: cx,cy,cz,r, ar,ag,ab, emissive(0/1) */ } gq_rt_scene;
 typedef struct { uint64_t rays, queue_ops; double ms, total_ms; uint32_t threads, items; } gq_rt_stats;
 int rt_render(int kind, const gq_rt_scene* scene, float* d_rgb /* DEVICE H*W*3 */, gq_rt_stats* stats_out, void* stream);
+/* The same image through the paper's own work distribution ("each tile owns its own queue"): mode 1 creates one queue
+   per 16x16 tile, items are RAYS (pixel in tile | sample << 8 | bounce << 14).  Every thread block owns the tiles b, b + blocks,
+   ...; its warps pull rays from those queues, 8 lanes per queue and 4 queues per instruction (the address-matched WAVEFAA,
+   gq::enqueue / dequeue with kUniform = false), trace them and re-enqueue the bounce into the queue of the same tile.  The
+   image is bit-identical to mode 0 (same per-path arithmetic, RNG keyed by pixel, sample and bounce).  GQ_LFQ and
+   GQ_LFQ_DIRECT only (the kinds with per-thread records would need tiles x threads of them): others return GQ_E_INVAL. */
+typedef struct { uint32_t mode;      /* 0 = one work queue of tile items (rt_render), 1 = one queue per tile, items = rays */
+                 uint32_t reserved; } gq_rt_opts;
+int rt_render_ex(int kind, const gq_rt_scene* scene, float* d_rgb, const gq_rt_opts* opts, gq_rt_stats* stats_out, void* stream);
 
 /* Debug and fault-injection builds only (include/gq/detail/debug.cuh; paper_2606_01693_b200/build.py variants "dbg"
    and "mutants").  In the product build all three return GQ_E_INVAL and do nothing.

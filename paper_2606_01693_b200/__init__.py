@@ -81,6 +81,10 @@ class gq_rt_scene(C.Structure):
                 ("n_spheres", C.c_uint32), ("threads", C.c_uint32), ("seed", C.c_uint64), ("d_spheres", C.c_void_p)]
 
 
+class gq_rt_opts(C.Structure):
+    _fields_ = [("mode", C.c_uint32), ("reserved", C.c_uint32)]
+
+
 class gq_rt_stats(C.Structure):
     _fields_ = [("rays", C.c_uint64), ("queue_ops", C.c_uint64), ("ms", C.c_double), ("total_ms", C.c_double),
                 ("threads", C.c_uint32), ("items", C.c_uint32)]
@@ -93,7 +97,7 @@ HIST_DTYPE = np.dtype([("proc", "<u4"), ("op", "<u4"), ("arg", "<u4"), ("ret_sta
 SYMBOLS = ("queue_storage_bytes", "queue_create", "queue_create_ex", "queue_destroy", "queue_reset", "queue_prefill",
            "queue_drain", "queue_device_view", "queue_kind", "queue_max_coresident_threads", "run_balanced",
            "run_split", "run_faa_ceiling", "run_slot_atomic_ceiling", "run_warp_faa_probe", "run_funnel_probe", "queue_run_script",
-           "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "gq_last_cuda_error", "gq_version",
+           "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "rt_render_ex", "gq_last_cuda_error", "gq_version",
            "gq_dbg_sites", "gq_dbg_trace", "gq_set_mutation", "queue_debug_counters")
 
 
@@ -124,6 +128,7 @@ def _load(variant=""):
     L.bfs_run.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, P(gq_bfs_stats), C.c_void_p]
     L.bfs_run_ex.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, P(gq_bfs_opts), P(gq_bfs_stats), C.c_void_p]
     L.rt_render.argtypes = [C.c_int, P(gq_rt_scene), C.c_void_p, P(gq_rt_stats), C.c_void_p]
+    L.rt_render_ex.argtypes = [C.c_int, P(gq_rt_scene), C.c_void_p, P(gq_rt_opts), P(gq_rt_stats), C.c_void_p]
     L.gq_last_cuda_error.restype = C.c_char_p
     L.gq_version.restype = C.c_char_p
     L.gq_dbg_sites.argtypes = [C.c_void_p]
@@ -327,8 +332,12 @@ def bfs_run_ex(kind, d_rowptr, d_col, nv, src, d_dist, stream=None, **opts):
     return {n: getattr(st, n) for n, _ in st._fields_}
 
 
-def rt_render(kind, width, height, spp, max_bounce, n_spheres, d_spheres, seed, d_rgb, threads=0, stream=None):
+def rt_render(kind, width, height, spp, max_bounce, n_spheres, d_spheres, seed, d_rgb, threads=0, stream=None, mode=0):
+    """mode 0: one work queue of tile items (rt_render); mode 1: one queue per tile, items are rays (rt_render_ex)."""
     sc = gq_rt_scene(width, height, spp, max_bounce, n_spheres, threads, seed, d_spheres)
     st = gq_rt_stats()
-    _chk(lib.rt_render(kind, C.byref(sc), d_rgb, C.byref(st), stream), "rt_render")
+    if mode:
+        _chk(lib.rt_render_ex(kind, C.byref(sc), d_rgb, C.byref(gq_rt_opts(mode, 0)), C.byref(st), stream), "rt_render_ex")
+    else:
+        _chk(lib.rt_render(kind, C.byref(sc), d_rgb, C.byref(st), stream), "rt_render")
     return {n: getattr(st, n) for n, _ in st._fields_}

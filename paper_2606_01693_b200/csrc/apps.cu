@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <vector>
 
 #include "gq.h"
 #include "gq/queue.cuh"
@@ -326,6 +327,86 @@ struct RtArgs {
   float* rgb;
 };
 
+// One path, one bounce: camera ray (bounce 0) or the stored ray, nearest hit, shading, scatter.  Returns true iff the path
+// lives on (its next ray is in a.state); a path that ends writes its radiance.  Arithmetic and its order: DESIGN.md section 6.
+__device__ __forceinline__ bool rt_path_step(const RtArgs& a, const float4* s_sph0, const float4* s_sph1, uint64_t path, uint32_t px,
+                                             uint32_t py, uint32_t sample, uint32_t bounce) {
+  const float aspect = (float)a.width / (float)a.height;
+  const uint32_t pixel = py * a.width + px;
+  V3 o, d, T;
+  if (bounce == 0) {                                            // primary ray: pinhole camera, DESIGN.md section 6
+    const float u0 = rt_rnd(a.seed, pixel, sample, 0, 0), u1 = rt_rnd(a.seed, pixel, sample, 0, 1);
+    const float sx = (((float)px + u0) / (float)a.width) * 2.0f - 1.0f;
+    const float sy = 1.0f - (((float)py + u1) / (float)a.height) * 2.0f;
+    d = V3{sx * (0.36397023f * aspect), sy * 0.36397023f, -1.0f};
+    d = vdiv(d, sqrtf(vdot(d, d)));
+    o = V3{0.0f, 0.0f, 35.0f};
+    T = V3{1.0f, 1.0f, 1.0f};
+  } else {
+    const float* S = a.state + path;
+    o = V3{S[0], S[a.n_paths], S[2 * a.n_paths]};
+    d = V3{S[3 * a.n_paths], S[4 * a.n_paths], S[5 * a.n_paths]};
+    T = V3{S[6 * a.n_paths], S[7 * a.n_paths], S[8 * a.n_paths]};
+  }
+  float best_t = __int_as_float(0x7f800000);
+  int best = -1;
+  for (uint32_t i = 0; i < a.ns; ++i) {                         // brute force, ties -> lowest index
+    const float4 c = s_sph0[i];                                 // cx, cy, cz, r
+    const V3 oc = vsub(o, V3{c.x, c.y, c.z});
+    const float bq = vdot(oc, d);
+    const float cq = vdot(oc, oc) - c.w * c.w;
+    const float disc = bq * bq - cq;
+    if (disc < 0.0f) continue;
+    const float sq = sqrtf(disc);
+    float t = -bq - sq;
+    if (!(t > 1e-3f)) { t = -bq + sq; if (!(t > 1e-3f)) continue; }
+    if (t < best_t) { best_t = t; best = (int)i; }
+  }
+  V3 L = {0.0f, 0.0f, 0.0f};
+  bool ended = true;
+  if (best < 0) {
+    L = vmul(T, V3{0.7f, 0.8f, 1.0f});                           // background
+  } else {
+    const float4 c = s_sph0[best], m = s_sph1[best];            // m = ar, ag, ab, emissive
+    const V3 albedo = {m.x, m.y, m.z};
+    if (m.w != 0.0f) {
+      L = vmul(T, vscale(albedo, 4.0f));                        // emissive: 4 x albedo, path ends
+    } else {
+      T = vmul(T, albedo);
+      if (bounce != a.max_bounce) {                             // else absorbed at the depth limit
+        const V3 hp = vadd(o, vscale(d, best_t));
+        const V3 n = vdiv(vsub(hp, V3{c.x, c.y, c.z}), c.w);
+        V3 unit = n;
+        for (uint32_t k = 0; k < 16; ++k) {                     // rejection sampling in the unit ball
+          const V3 v = {2.0f * rt_rnd(a.seed, pixel, sample, bounce, 2 + 3 * k) - 1.0f,
+                        2.0f * rt_rnd(a.seed, pixel, sample, bounce, 3 + 3 * k) - 1.0f,
+                        2.0f * rt_rnd(a.seed, pixel, sample, bounce, 4 + 3 * k) - 1.0f};
+          const float l2 = vdot(v, v);
+          if (l2 <= 1.0f && l2 > 1e-12f) { unit = vdiv(v, sqrtf(l2)); break; }
+        }
+        V3 sdir = vadd(n, unit);
+        float l2 = vdot(sdir, sdir);
+        if (!(l2 > 1e-12f)) { sdir = n; l2 = vdot(n, n); }
+        d = vdiv(sdir, sqrtf(l2));
+        o = hp;
+        ended = false;
+      }
+    }
+  }
+  if (ended) {
+    float* R = a.radiance + path;
+    R[0] = L.x; R[a.n_paths] = L.y; R[2 * a.n_paths] = L.z;
+    a.alive[path] = 0;
+    return false;
+  }
+  float* S = a.state + path;
+  S[0] = o.x; S[a.n_paths] = o.y; S[2 * a.n_paths] = o.z;
+  S[3 * a.n_paths] = d.x; S[4 * a.n_paths] = d.y; S[5 * a.n_paths] = d.z;
+  S[6 * a.n_paths] = T.x; S[7 * a.n_paths] = T.y; S[8 * a.n_paths] = T.z;
+  a.alive[path] = 1;
+  return true;
+}
+
 // Advance the (pixel, sample) paths of one item by one bounce.  Returns true iff any path lives on.
 __device__ __forceinline__ bool rt_advance(const RtArgs& a, const float4* s_sph0, const float4* s_sph1, uint32_t item, uint32_t lane,
                                            uint32_t& rays) {
@@ -334,88 +415,15 @@ __device__ __forceinline__ bool rt_advance(const RtArgs& a, const float4* s_sph0
   const uint32_t bounce = item >> (kItemTileBits + kItemSampleBits);
   const uint32_t tx = tile % a.tiles_x, ty = tile / a.tiles_x;
   const uint64_t path0 = ((uint64_t)tile * a.spp + sample) * kTilePixels;
-  const float aspect = (float)a.width / (float)a.height;
   bool any_alive = false;
   for (uint32_t j = 0; j < kPerLane; ++j) {
     const uint32_t p = lane + 32 * j;
     const uint32_t px = tx * kTile + (p % kTile), py = ty * kTile + (p / kTile);
     if (px >= a.width || py >= a.height) continue;
     const uint64_t path = path0 + p;
-    const uint32_t pixel = py * a.width + px;
-    V3 o, d, T;
-    if (bounce == 0) {                                            // primary ray: pinhole camera, DESIGN.md §6
-      const float u0 = rt_rnd(a.seed, pixel, sample, 0, 0), u1 = rt_rnd(a.seed, pixel, sample, 0, 1);
-      const float sx = (((float)px + u0) / (float)a.width) * 2.0f - 1.0f;
-      const float sy = 1.0f - (((float)py + u1) / (float)a.height) * 2.0f;
-      d = V3{sx * (0.36397023f * aspect), sy * 0.36397023f, -1.0f};
-      d = vdiv(d, sqrtf(vdot(d, d)));
-      o = V3{0.0f, 0.0f, 35.0f};
-      T = V3{1.0f, 1.0f, 1.0f};
-    } else {
-      if (!a.alive[path]) continue;
-      const float* S = a.state + path;
-      o = V3{S[0], S[a.n_paths], S[2 * a.n_paths]};
-      d = V3{S[3 * a.n_paths], S[4 * a.n_paths], S[5 * a.n_paths]};
-      T = V3{S[6 * a.n_paths], S[7 * a.n_paths], S[8 * a.n_paths]};
-    }
+    if (bounce != 0 && !a.alive[path]) continue;
     ++rays;
-    float best_t = __int_as_float(0x7f800000);
-    int best = -1;
-    for (uint32_t i = 0; i < a.ns; ++i) {                         // brute force, ties -> lowest index
-      const float4 c = s_sph0[i];                                 // cx, cy, cz, r
-      const V3 oc = vsub(o, V3{c.x, c.y, c.z});
-      const float bq = vdot(oc, d);
-      const float cq = vdot(oc, oc) - c.w * c.w;
-      const float disc = bq * bq - cq;
-      if (disc < 0.0f) continue;
-      const float sq = sqrtf(disc);
-      float t = -bq - sq;
-      if (!(t > 1e-3f)) { t = -bq + sq; if (!(t > 1e-3f)) continue; }
-      if (t < best_t) { best_t = t; best = (int)i; }
-    }
-    V3 L = {0.0f, 0.0f, 0.0f};
-    bool ended = true;
-    if (best < 0) {
-      L = vmul(T, V3{0.7f, 0.8f, 1.0f});                           // background
-    } else {
-      const float4 c = s_sph0[best], m = s_sph1[best];            // m = ar, ag, ab, emissive
-      const V3 albedo = {m.x, m.y, m.z};
-      if (m.w != 0.0f) {
-        L = vmul(T, vscale(albedo, 4.0f));                        // emissive: 4 x albedo, path ends
-      } else {
-        T = vmul(T, albedo);
-        if (bounce != a.max_bounce) {                             // else absorbed at the depth limit
-          const V3 hp = vadd(o, vscale(d, best_t));
-          const V3 n = vdiv(vsub(hp, V3{c.x, c.y, c.z}), c.w);
-          V3 unit = n;
-          for (uint32_t k = 0; k < 16; ++k) {                     // rejection sampling in the unit ball
-            const V3 v = {2.0f * rt_rnd(a.seed, pixel, sample, bounce, 2 + 3 * k) - 1.0f,
-                          2.0f * rt_rnd(a.seed, pixel, sample, bounce, 3 + 3 * k) - 1.0f,
-                          2.0f * rt_rnd(a.seed, pixel, sample, bounce, 4 + 3 * k) - 1.0f};
-            const float l2 = vdot(v, v);
-            if (l2 <= 1.0f && l2 > 1e-12f) { unit = vdiv(v, sqrtf(l2)); break; }
-          }
-          V3 sdir = vadd(n, unit);
-          float l2 = vdot(sdir, sdir);
-          if (!(l2 > 1e-12f)) { sdir = n; l2 = vdot(n, n); }
-          d = vdiv(sdir, sqrtf(l2));
-          o = hp;
-          ended = false;
-        }
-      }
-    }
-    if (ended) {
-      float* R = a.radiance + path;
-      R[0] = L.x; R[a.n_paths] = L.y; R[2 * a.n_paths] = L.z;
-      a.alive[path] = 0;
-    } else {
-      float* S = a.state + path;
-      S[0] = o.x; S[a.n_paths] = o.y; S[2 * a.n_paths] = o.z;
-      S[3 * a.n_paths] = d.x; S[4 * a.n_paths] = d.y; S[5 * a.n_paths] = d.z;
-      S[6 * a.n_paths] = T.x; S[7 * a.n_paths] = T.y; S[8 * a.n_paths] = T.z;
-      a.alive[path] = 1;
-      any_alive = true;
-    }
+    any_alive |= rt_path_step(a, s_sph0, s_sph1, path, px, py, sample, bounce);
   }
   return __any_sync(0xffffffffu, any_alive);
 }
@@ -580,7 +588,164 @@ int rt_render_t(const gq_rt_scene& sc, float* d_rgb, gq_rt_stats* st_out, cudaSt
   return 0;
 }
 
+// ---- mode 1: one queue per tile, items are rays ("each tile owns its own queue") ---------------------------------
+// Block b owns the tiles b, b + gridDim.x, ...  All of its warps serve those queues: in every round a warp looks at four
+// consecutive tiles of the block's list, 8 lanes per tile, so that the lanes converged at one enqueue / dequeue name up to four
+// different queues (kUniform = false: WAVEFAA elects one leader per queue inside the converged warp).  A lane that receives
+// a ray advances that path by one bounce and puts the next ray into the queue of the same tile.  s_pending counts the rays
+// of the block that are queued or in flight; the block is done when it reaches 0.  No grid-wide synchronisation.
+constexpr uint32_t kRayPixelBits = 8, kRaySampleBits = 6;
+template <class Q>
+__global__ void __launch_bounds__(256) rt_tiles_kernel(const Q* __restrict__ views, RtArgs a) {
+  __shared__ float4 s_sph0[kMaxSpheres];
+  __shared__ float4 s_sph1[kMaxSpheres];
+  __shared__ unsigned long long s_pending;
+  __shared__ uint32_t s_error;
+  for (uint32_t i = threadIdx.x; i < a.ns; i += blockDim.x) {
+    const float* S = a.spheres + 8 * i;
+    s_sph0[i] = make_float4(S[0], S[1], S[2], S[3]);
+    s_sph1[i] = make_float4(S[4], S[5], S[6], S[7]);
+  }
+  if (threadIdx.x == 0) { s_pending = 0; s_error = 0; }
+  __syncthreads();
+  const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  const uint32_t n_tiles = a.tiles_x * a.tiles_y;
+  const uint32_t my_tiles = blockIdx.x < n_tiles ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;   // tiles b, b + grid, ...
+  thread_ctx ctx{threadIdx.x};                                       // every tile queue is created for blockDim.x threads
+  uint32_t rays = 0, n_enq = 0, n_deq = 0;
+  // "Primary rays are generated and enqueued": (pixel, sample, bounce 0) of every tile the block owns
+  for (uint32_t i = threadIdx.x; i < my_tiles * a.spp * kTilePixels; i += blockDim.x) {
+    const uint32_t k = i / (a.spp * kTilePixels), r = i % (a.spp * kTilePixels), sample = r / kTilePixels, p = r % kTilePixels;
+    const uint32_t tile = blockIdx.x + k * gridDim.x;
+    const uint32_t px = (tile % a.tiles_x) * kTile + p % kTile, py = (tile / a.tiles_x) * kTile + p / kTile;
+    if (px >= a.width || py >= a.height) continue;
+    atomicAdd(&s_pending, 1ull);
+    if (enqueue<false, 1>(views[tile], ctx, p | sample << kRayPixelBits) != OK) { s_error = 1; atomicAdd(&s_pending, ~0ull); } else ++n_enq;
+  }
+  __threadfence();
+  __syncthreads();
+  for (uint32_t round = wib; my_tiles != 0; round += nwarps) {
+    if (*reinterpret_cast<volatile unsigned long long*>(&s_pending) == 0 || *reinterpret_cast<volatile uint32_t*>(&s_error)) break;
+    const uint32_t k = (round * 4 + (lane >> 3)) % my_tiles;         // four tiles per warp and round, 8 lanes each
+    const uint32_t tile = blockIdx.x + k * gridDim.x;
+    const Q& q = views[tile];
+    uint32_t item = 0;
+    if (dequeue<false, 1>(q, ctx, &item) != OK) continue;
+    ++n_deq;
+    const uint32_t p = item & ((1u << kRayPixelBits) - 1), sample = (item >> kRayPixelBits) & ((1u << kRaySampleBits) - 1);
+    const uint32_t bounce = item >> (kRayPixelBits + kRaySampleBits);
+    const uint32_t px = (tile % a.tiles_x) * kTile + p % kTile, py = (tile / a.tiles_x) * kTile + p / kTile;
+    const uint64_t path = ((uint64_t)tile * a.spp + sample) * kTilePixels + p;
+    ++rays;
+    if (rt_path_step(a, s_sph0, s_sph1, path, px, py, sample, bounce)) {
+      __threadfence();                                               // the path's next ray is visible before its item (queue.cuh, G15)
+      if (enqueue<false, 1>(q, ctx, item + (1u << (kRayPixelBits + kRaySampleBits))) != OK) { s_error = 1; atomicAdd(&s_pending, ~0ull); } else ++n_enq;
+    } else {
+      atomicAdd(&s_pending, ~0ull);
+    }
+  }
+  __syncwarp();
+  const uint64_t r = warp_sum64(rays), e = warp_sum64(n_enq), dq = warp_sum64(n_deq);
+  if (lane == 0) {
+    if (r) red_add_relaxed(a.ctr + R_RAYS, r);
+    if (e) red_add_relaxed(a.ctr + R_ENQ, e);
+    if (dq) red_add_relaxed(a.ctr + R_DEQ, dq);
+  }
+  if (threadIdx.x == 0 && s_error) st_relaxed(a.ctr + R_ERROR, 1);
+}
+
+template <class Q>
+int rt_render_tiles_t(const gq_rt_scene& sc, float* d_rgb, gq_rt_stats* st_out, cudaStream_t stream) {
+  const auto t_begin = std::chrono::steady_clock::now();
+  const int sms = gq_device_sms();
+  if (sms <= 0) { gq_set_error("no CUDA device"); return GQ_E_CUDA; }
+  RtArgs a{};
+  a.width = sc.width; a.height = sc.height; a.spp = sc.spp; a.max_bounce = sc.max_bounce; a.ns = sc.n_spheres;
+  a.seed = sc.seed; a.spheres = sc.d_spheres; a.rgb = d_rgb;
+  a.tiles_x = (sc.width + kTile - 1) / kTile; a.tiles_y = (sc.height + kTile - 1) / kTile;
+  const uint64_t tiles = (uint64_t)a.tiles_x * a.tiles_y;
+  if (tiles >= (1u << kItemTileBits) || sc.spp == 0 || sc.spp >= (1u << kRaySampleBits) || sc.max_bounce >= 60 ||
+      sc.n_spheres > kMaxSpheres || (sc.n_spheres && !sc.d_spheres) || (uint64_t)sc.width * sc.height >= (1ull << 31))
+    return GQ_E_INVAL;
+  a.n_items = (uint32_t)(tiles * sc.spp);
+  a.n_paths = (uint64_t)a.n_items * kTilePixels;
+  const uint32_t block = 256;
+  int nb = 0;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, rt_tiles_kernel<Q>, (int)block, 0));
+  if (nb <= 0) return GQ_E_CUDA;
+  uint32_t blocks = (uint32_t)nb * sms;
+  if (sc.threads) blocks = std::min(blocks, std::max(1u, sc.threads / block));
+  blocks = (uint32_t)std::min<uint64_t>(blocks, tiles);
+
+  gq_opts qo{};
+  qo.max_threads = block;                                 // a tile queue is served by the threads of one block
+  qo.park_ns = 20000;
+  qo.flags = GQ_F_EAGER_EMPTY | GQ_F_NO_FULL_TEST;        // polling consumers; a tile never holds more than 256 x spp rays
+  std::vector<gq_queue*> qs(tiles);
+  void* qblock = nullptr;
+  int rc = gq_create_many(ViewOf<Q>::kind, pow2ceil64((uint64_t)kTilePixels * sc.spp), &qo, (uint32_t)tiles, qs.data(), &qblock, stream);
+  if (rc) return rc;
+  std::vector<Q> h_views(tiles);
+  for (uint64_t i = 0; i < tiles && rc == 0; ++i) rc = queue_device_view(qs[i], &h_views[i], sizeof(Q));
+
+  char* scratch = nullptr;
+  const size_t ctr_bytes = 256, state_bytes = (size_t)a.n_paths * 9 * 4, rad_bytes = (size_t)a.n_paths * 3 * 4;
+  const size_t alive_bytes = (a.n_paths + 255) / 256 * 256, view_bytes = tiles * sizeof(Q);
+  cudaError_t e = rc ? cudaSuccess : cudaMalloc(&scratch, ctr_bytes + state_bytes + rad_bytes + alive_bytes + view_bytes);
+  if (rc || e != cudaSuccess) { gq_destroy_many(qs.data(), (uint32_t)tiles, qblock); return rc ? rc : gq_cuda_fail(e, "cudaMalloc(rt)"); }
+  a.ctr = reinterpret_cast<uint64_t*>(scratch);
+  a.state = reinterpret_cast<float*>(scratch + ctr_bytes);
+  a.radiance = reinterpret_cast<float*>(scratch + ctr_bytes + state_bytes);
+  a.alive = reinterpret_cast<uint8_t*>(scratch + ctr_bytes + state_bytes + rad_bytes);
+  Q* d_views = reinterpret_cast<Q*>(scratch + ctr_bytes + state_bytes + rad_bytes + alive_bytes);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  auto cleanup = [&]() { if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); cudaFree(scratch); gq_destroy_many(qs.data(), (uint32_t)tiles, qblock); };
+  e = cudaMemsetAsync(a.ctr, 0, ctr_bytes, stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_views, h_views.data(), view_bytes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(a.radiance, 0, rad_bytes, stream);
+  if (e == cudaSuccess) e = cudaEventCreate(&e0);
+  if (e == cudaSuccess) e = cudaEventCreate(&e1);
+  if (e == cudaSuccess) e = cudaEventRecord(e0, stream);
+  if (e != cudaSuccess) { cleanup(); return gq_cuda_fail(e, "rt setup"); }
+  rt_tiles_kernel<Q><<<blocks, block, 0, stream>>>(d_views, a);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) { cleanup(); return gq_cuda_fail(e, "rt launch"); }
+  const uint32_t npix = sc.width * sc.height;
+  rt_resolve_kernel<<<(npix + 255) / 256, 256, 0, stream>>>(a);
+  cudaEventRecord(e1, stream);
+  rc = gq_wait_event(e1, gq_watchdog_slack_s());
+  if (rc == GQ_E_TIMEOUT) return rc;                      // kernel still running: freeing would block on it
+  uint64_t c[R_COUNT] = {};
+  float ms = 0;
+  if (rc == 0) {
+    e = cudaMemcpy(c, a.ctr, sizeof c, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e != cudaSuccess) rc = gq_cuda_fail(e, "rt results");
+  }
+  cleanup();
+  if (rc) return rc;
+  if (c[R_ERROR]) return GQ_E_STATE;
+  if (st_out) {
+    gq_rt_stats s{};
+    s.rays = c[R_RAYS]; s.queue_ops = c[R_ENQ] + c[R_DEQ]; s.ms = ms; s.threads = blocks * block; s.items = (uint32_t)tiles;
+    s.total_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    *st_out = s;
+  }
+  return 0;
+}
+
 }  // namespace
+
+extern "C" int rt_render_ex(int kind, const gq_rt_scene* scene, float* d_rgb, const gq_rt_opts* opts, gq_rt_stats* stats_out, void* stream) {
+  if (!opts || opts->mode == 0) return rt_render(kind, scene, d_rgb, stats_out, stream);
+  if (!scene || !d_rgb || scene->width == 0 || scene->height == 0 || opts->mode != 1 || opts->reserved) return GQ_E_INVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  switch (kind) {
+    case GQ_LFQ: return rt_render_tiles_t<LfqView>(*scene, d_rgb, stats_out, st);
+    case GQ_LFQ_DIRECT: return rt_render_tiles_t<DlfqView>(*scene, d_rgb, stats_out, st);
+    default: return GQ_E_INVAL;                            // per-thread records x thousands of queues: see gq.h
+  }
+}
 
 extern "C" int rt_render(int kind, const gq_rt_scene* scene, float* d_rgb, gq_rt_stats* stats_out, void* stream) {
   if (!scene || !d_rgb || scene->width == 0 || scene->height == 0) return GQ_E_INVAL;

@@ -359,6 +359,46 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
 }
 extern "C" int queue_create(int kind, uint64_t capacity, gq_queue** out) { return queue_create_ex(kind, capacity, nullptr, out); }
 
+// `count` queues of the same shape in ONE device block, formatted on `stream` with one synchronisation at the end (the
+// per-tile queues of the multi-queue tracer: thousands of small queues).  G-LFQ / G-LFQ-D only: the kinds with
+// per-thread records would need count x max_threads of them.  Handles carry no run counters (no run_* on them).
+int gq_create_many(int kind, uint64_t capacity, const gq_opts* opts, uint32_t count, gq_queue** out, void** block_out, cudaStream_t st) {
+  if (!out || !block_out || count == 0 || (kind != GQ_LFQ && kind != GQ_LFQ_DIRECT) || (opts && opts->storage)) return GQ_E_INVAL;
+  Layout L; uint32_t k = 0;
+  int rc = compute_layout(kind, capacity, opts, &L, &k);
+  if (rc) return rc;
+  char* block = nullptr;
+  CU(cudaMalloc(&block, L.total * count));
+  for (uint32_t i = 0; i < count; ++i) out[i] = nullptr;
+  for (uint32_t i = 0; i < count && rc == 0; ++i) {
+    gq_queue* q = new (std::nothrow) gq_queue();
+    if (!q) { rc = GQ_E_NOMEM; break; }
+    out[i] = q;
+    q->kind = kind; q->capacity = capacity; q->N = L.N; q->max_threads = k; q->bytes = L.total;
+    if (opts) q->opts = *opts;
+    q->opts.flags &= kPublicFlags;
+    q->base = block + (size_t)i * L.total;
+    if (kind == GQ_LFQ_DIRECT) {
+      q->dlfq.r = make_ring(q->base, L, L.off_aq, 0, 0);
+      q->dlfq.capacity = (uint32_t)capacity; q->dlfq.flags = q->opts.flags;
+    } else {
+      q->lfq.aq = make_ring(q->base, L, L.off_aq, 0, 0);
+      q->lfq.fq = make_ring(q->base, L, L.off_fq, 0, 3);
+      q->lfq.data = reinterpret_cast<uint64_t*>(q->base + L.off_data);
+      q->lfq.capacity = (uint32_t)capacity; q->lfq.flags = q->opts.flags;
+    }
+    rc = format_queue(q, st);
+  }
+  if (rc == 0) { cudaError_t e = cudaStreamSynchronize(st); if (e != cudaSuccess) rc = cuda_fail(e, "format"); }
+  if (rc) { for (uint32_t i = 0; i < count; ++i) delete out[i]; cudaFree(block); return rc; }
+  *block_out = block;
+  return 0;
+}
+void gq_destroy_many(gq_queue** qs, uint32_t count, void* block) {
+  for (uint32_t i = 0; i < count; ++i) delete qs[i];
+  if (block) cudaFree(block);
+}
+
 extern "C" int queue_destroy(gq_queue* q) {
   if (!q) return GQ_E_INVAL;
   if (q->owns && q->base) cudaFree(q->base);

@@ -109,10 +109,10 @@ def test_bfs_rejects_bad_arguments():
 
 
 # ------------------------------------------------------------------------------------- tracer
-def render(kind, w, h, spp, bounces, spheres, seed, threads=0):
+def render(kind, w, h, spp, bounces, spheres, seed, threads=0, mode=0):
     d_sph = torch.from_numpy(np.ascontiguousarray(spheres, np.float32)).cuda() if len(spheres) else torch.zeros(8, device="cuda")
     d_rgb = torch.full((h, w, 3), -1.0, dtype=torch.float32, device="cuda")
-    st = gq.rt_render(kind, w, h, spp, bounces, len(spheres), d_sph.data_ptr(), seed, d_rgb.data_ptr(), threads=threads)
+    st = gq.rt_render(kind, w, h, spp, bounces, len(spheres), d_sph.data_ptr(), seed, d_rgb.data_ptr(), threads=threads, mode=mode)
     torch.cuda.synchronize()
     return d_rgb.cpu().numpy(), st
 
@@ -165,3 +165,42 @@ def test_rt_full_size_config5():
     ref, rays = oracle.rt_render(1920, 1080, 4, 4, sph, seed=1)
     check_image(img, ref)
     assert st["rays"] == rays and st["items"] == 8160 * 4
+
+
+# ---------------------------------------------------------------- one queue per tile, items are rays
+@pytest.mark.parametrize("kind", [gq.GQ_LFQ, gq.GQ_LFQ_DIRECT], ids=["G-LFQ", "G-LFQ-D"])
+def test_rt_per_tile_queues_small_ragged_image(kind):
+    sph = inputs.sphere_scene(64, seed=4)
+    img, st = render(kind, 150, 90, 2, 4, sph, seed=7, mode=1)
+    ref, rays = oracle.rt_render(150, 90, 2, 4, sph, seed=7)
+    exact = check_image(img, ref)
+    assert exact >= 0.999
+    assert st["rays"] == rays and st["queue_ops"] == 2 * rays          # every ray: one enqueue, one dequeue, in its tile's queue
+    assert st["items"] == 10 * 6                                        # one queue per tile
+    one, _ = render(kind, 150, 90, 2, 4, sph, seed=7, mode=0)
+    assert np.array_equal(img, one)                                     # the work distribution does not change a bit
+    few, _ = render(kind, 150, 90, 2, 4, sph, seed=7, mode=1, threads=512)   # 2 blocks share the 60 tiles
+    assert np.array_equal(img, few)
+
+
+def test_rt_per_tile_queues_closed_forms_and_kinds():
+    bg = np.array([0.7, 0.8, 1.0], np.float32)
+    img, st = render(gq.GQ_LFQ, 64, 48, 4, 4, np.zeros((0, 8), np.float32), seed=5, mode=1)
+    assert np.array_equal(img, np.broadcast_to(bg, img.shape)) and st["rays"] == 64 * 48 * 4
+    sph = np.array([[0, 0, 0, 5, 0.25, 0.5, 0.75, 1]], np.float32)
+    img, _ = render(gq.GQ_LFQ, 96, 64, 1, 4, sph, seed=9, mode=1)
+    hit = (img == np.array([1.0, 2.0, 3.0], np.float32)).all(axis=2)
+    assert (hit | (img == bg).all(axis=2)).all() and hit[32, 48] and not hit[0, 0]
+    for kind in (gq.GQ_WFQ, gq.GQ_WFQ_YMC):                              # per-thread records x thousands of queues: refused
+        with pytest.raises(gq.GqError):
+            render(kind, 64, 48, 1, 1, sph, seed=1, mode=1)
+
+
+def test_rt_per_tile_queues_full_size_config5():
+    # BASELINE.json config 5 through 8160 tile queues
+    sph = inputs.sphere_scene(256, seed=1)
+    img, st = render(gq.GQ_LFQ, 1920, 1080, 4, 4, sph, seed=1, mode=1)
+    one, st0 = render(gq.GQ_LFQ, 1920, 1080, 4, 4, sph, seed=1, mode=0)
+    assert np.array_equal(img, one)                                     # test_rt_full_size_config5 compares mode 0 with the oracle
+    assert st["rays"] == st0["rays"] and st["items"] == 8160
+    print(f"\n[rt] 1920x1080: one queue {st0['ms']:.2f} ms, 8160 tile queues {st['ms']:.2f} ms (setup {st['total_ms'] - st['ms']:.0f} ms)")
