@@ -42,9 +42,13 @@ ALGO_BYTES_PER_OP = {"lfq": 36.5, "wfq": 37.0, "ymc": 12.0, "lfq_direct": 12.5}
 IMPL_EXTRA_BYTES_PER_OP = {"lfq": 4.0, "wfq": 4.0, "ymc": 4.0, "lfq_direct": 0.0}
 CEILING_WINDOWS, CEILING_MS = 5, 100.0     # every ceiling: median of 5 windows of 100 ms, spread reported
 KINDS = {"lfq": 0, "wfq": 1, "ymc": 2, "lfq_direct": 3}   # lfq_direct: ablation kind (include/gq/dlfq.cuh), sweep context only
-# G-WFQ-YMC never reuses a cell: a 120 ms run at ~25 Gops/s touches ~1.5 G cells, so
-# the timed runs get a 2^32-cell pool (64 GiB of the 180 GB HBM); the other kinds ignore the field.
-YMC_POOL_CELLS = 1 << 32
+# G-WFQ-YMC's pool is a ring (Y10): 0 = the default size pow2ceil(capacity + 4k) = 2^20 cells (16 MiB) for BJ#2,
+# 2^21 for BJ#3; every cell is reused every ~45 us of a timed run.  The other kinds ignore the field.
+YMC_POOL_CELLS = 0
+# The lanes of a warp start every iteration of the benchmark loop together (gq_run_cfg.converged), as the lock-step
+# wavefronts of the paper's kernels do: without it a warp that has split once stays split for the rest of the
+# launch and draws partial WAVEFAA batches (the two steady states of round 1: 62 vs 79 Gops/s at n >= 2^18).
+CONVERGED = 1
 
 
 def env_int(name, default):
@@ -201,6 +205,19 @@ def run_apps(gq, torch, scale, fast_oracle=True):
                     "queue_Mops": round(best["queue_ops"] / (best["ms"] * 1e-3) / 1e6, 3), "items": best["items"],
                     "pixels_within_1e-3": float((err <= 1e-3).mean()), "pixels_bit_exact": float((err == 0).mean()),
                     "rays_match_oracle": bool(best["rays"] == ref_rays)}
+    # the paper's own work distribution: one queue per tile, items are rays; must reproduce the image bit for bit
+    best = None
+    one = d_rgb.clone()
+    gq.rt_render(0, W, H, SPP, B, len(sph), d_sph.data_ptr(), 1, one.data_ptr())
+    for _ in range(3):
+        st = gq.rt_render(0, W, H, SPP, B, len(sph), d_sph.data_ptr(), 1, d_rgb.data_ptr(), mode=1)
+        torch.cuda.synchronize()
+        if best is None or st["ms"] < best["ms"]:
+            best = st
+    rt["lfq_one_queue_per_tile"] = {"ms": round(best["ms"], 3), "total_ms": round(best["total_ms"], 3), "queues": best["items"],
+                                    "Mrays": round(best["rays"] / (best["ms"] * 1e-3) / 1e6, 1),
+                                    "queue_Mops": round(best["queue_ops"] / (best["ms"] * 1e-3) / 1e6, 1),
+                                    "identical_to_single_queue": bool(torch.equal(one, d_rgb))}
     out["rt"] = rt
     return out
 
@@ -225,7 +242,7 @@ def run_ours(args, rank, world, local_rank):
     threads = args.threads or full
     q = gq.queue_create_ex(kind, CAPACITY, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-    run_kw = dict(threads=threads, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns)
+    run_kw = dict(threads=threads, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns, converged=CONVERGED)
 
     def barrier():
         torch.cuda.synchronize()
@@ -331,7 +348,7 @@ def run_ours(args, rank, world, local_rank):
                 gq.queue_reset(qs)
                 gq.queue_prefill(qs, pre)
                 r = gq.run_split(qs, threads=threads, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=0.5, seed=1,
-                                 value_base=1 << 19, role_layout=layout)
+                                 value_base=1 << 19, role_layout=layout, converged=CONVERGED)
                 xs.append((r["succ_enq"] + r["succ_deq"]) / r["meas_seconds"])
             runs[layout] = xs
         gq.queue_destroy(qs)
@@ -357,7 +374,7 @@ def run_ours(args, rank, world, local_rank):
             pts = {}
             for th in (32, 256, 2048, 16384, 65536, fk):
                 gq.queue_reset(qq)
-                r = gq.run_balanced(qq, threads=th, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns)
+                r = gq.run_balanced(qq, threads=th, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, fail_backoff_ns=args.fail_backoff_ns, converged=CONVERGED)
                 pts[str(th)] = round(r["mops"], 1)
                 if r["pool_exhausted"]:
                     pts[str(th) + "_pool_exhausted"] = True      # G-WFQ-YMC ran out of cells inside the run: the number is low
@@ -371,7 +388,7 @@ def run_ours(args, rank, world, local_rank):
                     gq.queue_reset(qq)
                     gq.queue_prefill(qq, pre)
                     r = gq.run_split(qq, threads=fk, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=pf,
-                                     seed=1, value_base=1 << 19, fail_backoff_ns=args.fail_backoff_ns)
+                                     seed=1, value_base=1 << 19, fail_backoff_ns=args.fail_backoff_ns, converged=CONVERGED)
                     pts[str(pf)] = {"enq_mops": round(r["succ_enq"] / r["meas_seconds"] / 1e6, 1),
                                     "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1),
                                     "full_rate": round(r["full"] / max(1, r["full"] + r["succ_enq"]), 4),
@@ -382,7 +399,7 @@ def run_ours(args, rank, world, local_rank):
                         gq.queue_reset(qq)
                         gq.queue_prefill(qq, pre)
                         r = gq.run_split(qq, threads=fk, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=pf,
-                                         seed=1, value_base=1 << 19, role_layout=1)
+                                         seed=1, value_base=1 << 19, role_layout=1, converged=CONVERGED)
                         ptc[str(pf)] = {"enq_mops": round(r["succ_enq"] / r["meas_seconds"] / 1e6, 1),
                                         "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1)}
                     sweep["split_lfq_role_layout_1"] = ptc
@@ -392,16 +409,35 @@ def run_ours(args, rank, world, local_rank):
                 sweep["split_" + name] = str(e)
 
     if not args.no_sweep:
-        # capacity sweep at full co-residency (G-LFQ): for n < k the throughput is 2n / (index cycle), DESIGN.md section 5
+        # capacity sweep at full co-residency (G-LFQ): for n < k the throughput is 2n / (index cycle), DESIGN.md section 5;
+        # 5 runs per point: median, min, max (stability: the retry episodes and the two steady states of round 1)
         pts = {}
         for logn in (13, 14, 15, 16, 17, 18, 20):
             qq = gq.queue_create(0, 1 << logn)
-            r = gq.run_balanced(qq, threads=full, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS)
+            xs = []
+            for _ in range(5):
+                gq.queue_reset(qq)
+                xs.append(gq.run_balanced(qq, threads=full, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, converged=CONVERGED)["mops"])
             gq.queue_destroy(qq)
-            pts[f"2^{logn}"] = {"mops": round(r["mops"], 1), "index_cycle_us": round(2.0 * (1 << logn) / (r["mops"] * 1e6) * 1e6, 2) if (1 << logn) < full else None}
-        pts["note"] = ("n < k: ops/s = 2n / index cycle.  n = 2^17 is slightly below k = full: runs there can contain retry "
-                       "episodes (DESIGN.md section 5, open issue); n >= 2^18 settles in one of two steady states (62 or 79 Gops/s)")
+            med = statistics.median(xs)
+            pts[f"2^{logn}"] = {"mops": round(med, 1), "min": round(min(xs), 1), "max": round(max(xs), 1),
+                                "index_cycle_us": round(2.0 * (1 << logn) / (med * 1e6) * 1e6, 2) if (1 << logn) < full else None}
+        pts["note"] = "5 runs per point (median, min, max).  n < k: ops/s = 2n / index cycle; n >= 2^18 is bound by the four hot counters"
         sweep["capacity_lfq_full_coresidency"] = pts
+        # ablations at the headline point: free-running lanes (converged = 0), block-level ticket funnels (D11)
+        abl = {}
+        for name, k, n, kw in (("lfq_n2^16_free_running_lanes", 0, CAPACITY, dict(converged=0)),
+                               ("lfq_n2^20_free_running_lanes", 0, 1 << 20, dict(converged=0)),
+                               ("lfq_n2^20_block_funnels", 0, 1 << 20, dict(converged=1, block_faa=1)),
+                               ("ymc_n2^16_block_funnels_window_300ns", 2, CAPACITY, dict(converged=1, block_faa=1, funnel_window_ns=300))):
+            qq = gq.queue_create_ex(k, n, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
+            xs = []
+            for _ in range(3):
+                gq.queue_reset(qq)
+                xs.append(gq.run_balanced(qq, threads=full if k == 0 else gq.queue_max_coresident_threads(k, 256), warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, **kw)["mops"])
+            gq.queue_destroy(qq)
+            abl[name] = {"mops": round(statistics.median(xs), 1), "min": round(min(xs), 1), "max": round(max(xs), 1)}
+        sweep["ablations"] = abl
 
     apps = None
     if args.apps:
@@ -429,8 +465,8 @@ def run_ours(args, rank, world, local_rank):
         "warmup": args.warmup, "ms_per_step": wall_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": f"BJ#2 balanced fixed-duration: {args.kind} capacity 2^16 uint32, {threads} threads "
-                               f"(full co-residency = {full}), block 256, 20 ms warmup + 100 ms window per step",
-                   "kind": args.kind, "threads": threads, "capacity": CAPACITY, "fail_backoff_ns": args.fail_backoff_ns,
+                               f"(full co-residency = {full}), block 256, 20 ms warmup + 100 ms window per step, lanes of a warp start each iteration together",
+                   "kind": args.kind, "threads": threads, "capacity": CAPACITY, "fail_backoff_ns": args.fail_backoff_ns, "converged": CONVERGED,
                    "l2": "256 MiB device buffer written between steps (L2 flush); rings are L2-resident by design",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "e2e": {"value": e2e_ops_all / e2e_wall_max / 1e6, "unit": "Mops/s", "h2d_bytes_per_step": 64,   # the gq_run_cfg struct

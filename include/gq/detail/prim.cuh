@@ -149,7 +149,11 @@ __device__ __forceinline__ uint64_t funnel_faa(BlockFunnel* f, uint64_t* counter
   volatile unsigned int* vseq = &s->seq;
   volatile unsigned int* vreaders = &s->readers;
   if (place != 0) {                                                   // follow (the whole group)
-    while (*vseq != seq) __nanosleep(20);                             // the nap lets diverged lanes of this very warp run: the combiner may be one
+    [[maybe_unused]] uint32_t sn = 0;
+    while (*vseq != seq) {                                            // the nap lets diverged lanes of this very warp run: the combiner may be one
+      if (GQ_STUCK(sn, 50, seq, &f->gate, &s->base, &s->seq)) break;
+      __nanosleep(20);
+    }
     const uint64_t base = *reinterpret_cast<volatile unsigned long long*>(&s->base);
     if (lead) atomicSub(&s->readers, 1u);
     return base + (uint64_t)off * unit;
@@ -166,7 +170,11 @@ __device__ __forceinline__ uint64_t funnel_faa(BlockFunnel* f, uint64_t* counter
   if (lead && (blockIdx.x & 63u) == 0) { GQ_COUNT(22, 1); GQ_COUNT(23, warps); }   // funnel batches, groups per batch (sampled blocks)
 #endif
   {
-    while (*vseq != seq - kFunnelSlots || *vreaders != 0) __nanosleep(20);   // previous tenant of the slot published and read
+    [[maybe_unused]] uint32_t sn = 0;
+    while (*vseq != seq - kFunnelSlots || *vreaders != 0) {           // previous tenant of the slot published and read
+      if (GQ_STUCK(sn, 51, seq, &f->gate, &s->base, &s->seq)) break;
+      __nanosleep(20);
+    }
     if (lead) {
       *reinterpret_cast<volatile unsigned long long*>(&s->base) = base;
       *vreaders = warps - 1u;
@@ -186,7 +194,10 @@ __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 
 #endif
   const uint32_t leader = __ffs(mask) - 1;
   const uint32_t rank = __popc(mask & lanemask_lt()) + (GQ_MUT(MUT_RANK_OFF_BY_ONE) ? 1u : 0u);
-  if (funnel) return funnel_faa(funnel, counter, unit, mask, leader) + (uint64_t)rank * unit;   // all lanes of one group name one funnel
+  // Only a whole warp goes through the funnel: then no warp ever has two groups inside one (a follower and its combiner,
+  // or a combiner and a reader it waits for, in the same warp would depend on how the hardware interleaves diverged lanes);
+  // the stragglers of a diverged warp draw their tickets directly.
+  if (funnel && mask == 0xFFFFFFFFu) return funnel_faa(funnel, counter, unit, mask, leader) + (uint64_t)rank * unit;
   uint64_t base = 0;
   if (lane_id() == leader) {
     base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);

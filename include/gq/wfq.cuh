@@ -396,13 +396,19 @@ __device__ __forceinline__ void wfq_help_threads(const WfqView& q, thread_ctx& c
 
 }  // namespace detail
 
+// ring_enq / ring_deq are real functions shared by the AQ and the FQ side of both operations: lanes of one warp that have
+// drifted apart (one still in its enqueue, one already in its dequeue; the two roles of a mixed warp) can meet inside them
+// naming DIFFERENT rings, whatever the caller promised about the queue.  Inside G-WFQ the WAVEFAA therefore always groups
+// lanes by counter address (kUniform = false costs one match.any per ticket).
+constexpr bool kSameRing = false;
+
 template <bool kUniform = false, int kWarpFaa = true>
 __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32_t v, uint64_t* retries = nullptr) {
   using namespace detail;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   wfq_help_threads(q, ctx);
   uint32_t idx;
-  if (Wf::ring_deq<kUniform, kWarpFaa>(q.fq, &idx, q.deq_patience, ctx.tid, q.nthreads, retries, (ctx.hungry & 2u) != 0, q.flags) == RING_EMPTY) {
+  if (Wf::ring_deq<kSameRing, kWarpFaa>(q.fq, &idx, q.deq_patience, ctx.tid, q.nthreads, retries, (ctx.hungry & 2u) != 0, q.flags) == RING_EMPTY) {
     ctx.hungry |= 2u;
     return FULL;
   }
@@ -411,9 +417,9 @@ __device__ __forceinline__ int enqueue(const WfqView& q, thread_ctx& ctx, uint32
   uint64_t* cell = q.data + idx;
   if (q.flags & kFencedPayload) {                                   // the paper's scheme: payload, then release-install
     st_relaxed(cell, (uint64_t)v);
-    Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags);
+    Wf::ring_enq<kSameRing, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags);
   } else {
-    Wf::ring_enq<kUniform, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags, false, 0, cell, v);
+    Wf::ring_enq<kSameRing, kWarpFaa>(q.aq, idx, q.enq_patience, ctx.tid, retries, q.flags, false, 0, cell, v);
   }
   return OK;
 }
@@ -424,7 +430,7 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   wfq_help_threads(q, ctx);
   uint32_t idx;
-  if (Wf::ring_deq<kUniform, kWarpFaa>(q.aq, &idx, q.deq_patience, ctx.tid, q.nthreads, retries, (ctx.hungry & 1u) != 0, q.flags, &ctx.last_ticket) == RING_EMPTY) {
+  if (Wf::ring_deq<kSameRing, kWarpFaa>(q.aq, &idx, q.deq_patience, ctx.tid, q.nthreads, retries, (ctx.hungry & 1u) != 0, q.flags, &ctx.last_ticket) == RING_EMPTY) {
     ctx.hungry |= 1u;
     return EMPTY;
   }
@@ -438,12 +444,12 @@ __device__ __forceinline__ int dequeue(const WfqView& q, thread_ctx& ctx, uint32
   // delivered its value (control dependency), so the fast-path install needs no release fence.
   const bool paired = !(q.flags & kNoPairedFaa) && q.enq_patience != 0 && q.enq_patience != 0xFFFFFFFFu;
   uint64_t t = 0;
-  if (paired) t = Ring<WfqFmt, kUniform, kWarpFaa>::take(q.fq, false);
+  if (paired) t = Ring<WfqFmt, kSameRing, kWarpFaa>::take(q.fq, false);
   if (fast) w = cell_await(cell, w, ctx.last_ticket);               // tagged cell: wait for the store of THIS tenure of idx
   *out = (uint32_t)w;
   GQ_IDX_EVENT(7, q.aq, idx, ctx.last_ticket, w, fast);
   const uint32_t fl = (q.flags & kFencedPayload) ? q.flags : (q.flags | kRelaxedInstall);
-  Wf::ring_enq<kUniform, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, fl, paired, t);
+  Wf::ring_enq<kSameRing, kWarpFaa>(q.fq, idx, q.enq_patience, ctx.tid, retries, fl, paired, t);
   return OK;
 }
 

@@ -36,6 +36,9 @@ class GqError(RuntimeError):
         self.code = code
         if code == GQ_E_TIMEOUT:
             TIMED_OUT = True
+            if os.environ.get("GQ_EXIT_ON_TIMEOUT"):      # test runs: every later CUDA call (frees included) would block on the stuck kernel
+                os.write(2, f"\n[gq] {where}: watchdog time-out, kernel still running; exiting (GQ_EXIT_ON_TIMEOUT)\n".encode())
+                os._exit(3)
         detail = lib.gq_last_cuda_error().decode() if code in (GQ_E_CUDA, GQ_E_TIMEOUT, GQ_E_NOMEM) else ""
         super().__init__(f"{where}: GQ_E_{_ERR.get(code, code)} {detail}".strip())
 

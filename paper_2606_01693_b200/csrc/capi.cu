@@ -131,8 +131,9 @@ static int compute_layout(int kind, uint64_t capacity, const gq_opts* o, Layout*
       L->off_rec_fq = off; off += (size_t)k * sizeof(WfqRecord);
     }
   } else {
-    L->pool_cells = o->ymc_pool_cells ? o->ymc_pool_cells : (1ull << 26);    // reading Y3
-    if (L->pool_cells < 64 || L->pool_cells >= (1ull << 40)) return GQ_E_INVAL;
+    // the pool is a ring of P cells (Y10): P = pow2ceil(max(capacity + 4k, ymc_pool_cells)); FULL from P - 2k tickets on
+    if (k + 2 > Ymc::kIdTop || o->ymc_pool_cells >= (1ull << 40)) return GQ_E_INVAL;
+    L->pool_cells = pow2ceil(std::max<uint64_t>(std::max<uint64_t>(capacity + 4ull * k, o->ymc_pool_cells), 64));
     L->N = pow2ceil(k);
     L->off_rec = off; off += (size_t)k * sizeof(YmcHandle);
     L->off_pool = off; off += (size_t)L->pool_cells * sizeof(YmcCell);
@@ -207,25 +208,12 @@ __global__ void format_ymc_handles_kernel(YmcHandle* h, uint32_t n) {
   z.enq_peer = z.deq_peer = i + 1 < n ? i + 1 : 0;
   h[i] = z;
 }
-// T = H = 0, flag clear, and the sentinel cell at the end of the pool sealed (val = top, enq = top_e,
-// deq = top_d) so that a ticket past the pool can never deposit or claim anything.
-__global__ void format_ymc_words_kernel(YmcView q) {
-  *q.tail = 0; *q.head = 0; *q.exhausted = 0;
-  YmcCell* c = q.pool + (q.pool_cells - 1);
-  c->val = Ymc::kTop; c->enq = Ymc::kTop32; c->deq = Ymc::kTop32;
-}
+// T = H = 0 (all cells zero = <epoch 0, bot, bot_e, bot_d>, no payload tag)
+__global__ void format_ymc_words_kernel(YmcView q) { *q.tail = 0; *q.head = 0; *q.exhausted = 0; }
 
 static int format_queue(gq_queue* q, cudaStream_t st) {
   if (q->kind == GQ_WFQ_YMC) {
-    // only the cells tickets have reached can be dirty: zero [0, max(T, H) + k + 64)
-    uint64_t dirty = q->ymc.pool_cells;
-    if (q->formatted) {
-      uint64_t th[2] = {0, 0};
-      CU(cudaMemcpyAsync(&th[0], q->ymc.tail, 8, cudaMemcpyDeviceToHost, st));
-      CU(cudaMemcpyAsync(&th[1], q->ymc.head, 8, cudaMemcpyDeviceToHost, st));
-      CU(cudaStreamSynchronize(st));
-      dirty = std::min<uint64_t>(q->ymc.pool_cells, std::max(th[0], th[1]) + q->max_threads + 64);
-    }
+    const uint64_t dirty = q->ymc.pool_cells;
     CU(cudaMemsetAsync(q->ymc.pool, 0, (size_t)dirty * sizeof(YmcCell), st));
     format_ymc_handles_kernel<<<(q->max_threads + 255) / 256, 256, 0, st>>>(q->ymc.handles, q->max_threads);
     format_ymc_words_kernel<<<1, 1, 0, st>>>(q->ymc);
@@ -349,6 +337,8 @@ extern "C" int queue_create_ex(int kind, uint64_t capacity, const gq_opts* opts,
     q->ymc.park_ns = L.park_ns;
     q->ymc.park_nap = L.park_nap;
     q->ymc.park_limit = (uint32_t)std::min<uint64_t>(L.N / 2, 0x7FFFFFFFu);
+    q->ymc.pool_shift = 0; while ((1ull << q->ymc.pool_shift) < L.pool_cells) ++q->ymc.pool_shift;
+    q->ymc.full_limit = L.pool_cells - 2ull * k;
   }
   rc = format_queue(q, nullptr);
   q->fresh = rc == 0;

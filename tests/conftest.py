@@ -8,6 +8,9 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+os.environ.setdefault("GQ_EXIT_ON_TIMEOUT", "1")      # a watchdog time-out ends the test run at once (see paper_2606_01693_b200.GqError)
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
