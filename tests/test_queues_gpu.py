@@ -387,6 +387,71 @@ def test_medium_history_bad_pattern_check(kind, threads, ops, capacity):
     check_medium_history(kind, threads, ops, capacity, max_fail_returns=256)
 
 
+# ---------------------------------------------------------------- G-WFQ-YMC on a small pool: every cell reused over and over (Y10)
+Z = gq.GQ_PATIENCE_ZERO
+RING_OPTS = {"fast": {}, "p1": dict(enq_patience=1, deq_patience=1), "p0": dict(enq_patience=Z, deq_patience=Z)}
+
+
+@pytest.mark.parametrize("variant", list(RING_OPTS))
+def test_ymc_ring_pool_is_lapped_thousands_of_times(variant):
+    # capacity 64, 64 threads: the default pool is pow2ceil(64 + 4 * 64) = 512 cells, so 64 threads x 8192 iterations lap it
+    # a thousand times, slow paths and helpers included; conservation per launch, and afterwards the queue still works in order
+    q = gq.queue_create_ex(gq.GQ_WFQ_YMC, 64, gq.gq_opts(max_threads=64, **RING_OPTS[variant]))
+    try:
+        ops = 8192 if variant != "p0" else 1024
+        for rep in range(3):
+            r = gq.run_balanced(q, threads=64, block_threads=32, ops_per_thread=ops, value_base=rep * 64 * ops)
+            left = gq.queue_drain(q, 1024)
+            conserve(r, left)
+            assert r["tot_enq"] + r["tot_full"] == 64 * ops
+        c = gq.queue_debug_counters(q)
+        assert c["tail"] > 512 * (100 if variant != "p0" else 10)                     # many laps of the 512-cell pool
+        # split with homogeneous warps: consumers burn cells ahead of the producers, lap after lap
+        for rep in range(3):
+            r = gq.run_split(q, threads=64, block_threads=32, ops_per_thread=ops, producer_fraction=0.5, seed=3 + rep, role_layout=1,
+                             value_base=(3 + rep) * 64 * ops)
+            left = gq.queue_drain(q, 1024)
+            conserve(r, left)
+        gq.queue_prefill(q, np.arange(100, dtype=np.uint32))
+        assert np.array_equal(gq.queue_drain(q, 200), np.arange(100, dtype=np.uint32))
+    finally:
+        gq.queue_destroy(q)
+
+
+@pytest.mark.parametrize("variant", ["fast", "p1"])
+def test_ymc_ring_history_over_several_laps(variant):
+    # 64 threads x 128 iterations on the 512-cell pool: 16 384 recorded operations, 16 laps; OK / EMPTY histories with unique
+    # values: the bad-pattern characterisation is exact
+    q = gq.queue_create_ex(gq.GQ_WFQ_YMC, 64, gq.gq_opts(max_threads=64, **RING_OPTS[variant]))
+    try:
+        r = gq.run_balanced(q, threads=64, block_threads=32, ops_per_thread=128, record_history=1, jitter_ns=100, seed=5)
+        recs = gq.history_dump(q)
+        left = gq.queue_drain(q, 1024)
+    finally:
+        gq.queue_destroy(q)
+    assert len(recs) == 64 * 128 * 2 and r["tot_full"] == 0
+    h = to_history(recs)
+    assert oracle.precheck(h) == "" and oracle.conservation(h, left) == ""
+    pr, why = oracle.poly(h)
+    assert pr == oracle.LIN_OK, why
+
+
+def test_ymc_ring_full_is_the_pool():
+    # single thread: capacity 8, 32 threads -> pool 256 cells.  FULL appears when the ticket laps onto an unconsumed cell, i.e.
+    # after exactly 256 items (the soft bound: between n + 2k and P); FIFO order survives it, and so does the queue
+    q = gq.queue_create_ex(gq.GQ_WFQ_YMC, 8, gq.gq_opts(max_threads=32, park_ns=2000))
+    try:
+        n = 300
+        st, _ = gq.queue_run_script(q, np.zeros(n, np.uint32), np.arange(n, dtype=np.uint32), tid=3)
+        assert (st[:256] == gq.GQ_OK).all() and (st[256:] == gq.GQ_FULL).all()
+        out = gq.queue_drain(q, 1000)
+        assert np.array_equal(out, np.arange(256, dtype=np.uint32))
+        st, val = gq.queue_run_script(q, [0, 0, 1, 1, 1], [7, 8, 0, 0, 0], tid=3)
+        assert st.tolist() == [0, 0, 0, 0, gq.GQ_EMPTY] and val[2:4].tolist() == [7, 8]
+    finally:
+        gq.queue_destroy(q)
+
+
 # ---------------------------------------------------------------- block-level ticket funnels (D11)
 @pytest.mark.parametrize("kind", BIG)
 @pytest.mark.parametrize("window", [0, 300])
