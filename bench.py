@@ -322,7 +322,7 @@ def run_ours(args, rank, world, local_rank):
     roofline = {"bound": "l2_atomic", "achieved": ops_per_s_kernel / 1e9, "peak": 2 * c1_tps / 1e9, "unit": "Gop/s",
                 "frac": ops_per_s_kernel / (2 * c1_tps), "traffic": traffic,
                 "traffic_detail": traffic_detail, "traffic_note": "DRAM bytes of the committed ncu --set full capture of this kernel (fixed-op launch, "
-                "profiles/r1b_balanced_ncu_full.md): the rings are L2-resident, so DRAM sees the cold first touch only; L2 sector bytes per op beside it",
+                "profiles/r2_balanced_ncu_full.md): the rings are L2-resident, so DRAM sees the cold first touch only; L2 sector bytes per op beside it",
                 "kernel": "gqk::bench_kernel", "kernel_ms": kernel_ms,
                 "peak_source": "2 x C1; C1 = run_faa_ceiling(1 counter) at the same thread count, measured in this run (median of 5 x 100 ms)",
                 "c1_gtickets_s": c1_tps / 1e9, "c1_min_max": [c1_min / 1e9, c1_max / 1e9],

@@ -85,13 +85,19 @@ struct Wf {
     if (ld_relaxed(&p->p2_seq1) != s2) return;
     if (((target & 1) != 0) != kDeq && !GQ_MUT(MUT_P2_ANY_SIDE)) return;
     if ((expect >> S) >= c || !(expect & kINC)) return;
-    if (cas_acq_rel(local_ptr(r, target), expect, expect & ~kINC) == expect) {
+    if (cas_relaxed(local_ptr(r, target), expect, expect & ~kINC) == expect) {
       GQ_L_EVENT(r, target, 'P', me, expect, ((uint64_t)u << 44) | c);
       WfqRecord* mine = rec(r, me);
       ++((target & 1) ? mine->n_head_clr : mine->n_tail_clr);
     }
   }
 
+  // Memory orders of the slow path (sm_100a: an acq_rel atomic is MEMBAR.ALL.GPU + ATOM, about two L2 round trips).  Every
+  // word below is only ever accessed with L2 atomics and strong loads, and the protocol decides on VALUES (counters, tags,
+  // cycles), so most transitions are relaxed.  Two edges carry data and keep their order: (i) the phase-2 record goes out
+  // before the CAS that puts this thread's id into G (release; readers of the ThrIdx acquire G); (ii) the payload cell and
+  // the request record go out before the entry is installed (the helper acquires the record's sequence word, its
+  // installing CAS is a release, the dequeuer's slot load an acquire).
   // SLOWFAA (Alg. 2; reading W4).  G = global Head or Tail word, L = the request's
   // local word, v = last value of L this helper knows, tag = request tag, me = this thread.
   // Returns true with v = <ticket, tag> (no flags) when the round's ticket is known; false when
@@ -101,6 +107,7 @@ struct Wf {
                                   uint64_t target_id) {
     WfqRecord* mine = rec(r, me);
     uint64_t c = 0;
+    Backoff bo;
     [[maybe_unused]] uint32_t sn1 = 0, sn2 = 0;
     for (;;) {
       if (GQ_STUCK(sn1, (kDeq ? 11 : 10) | r.id << 8, me, G, L, kDeq ? r.tail : r.head, r.threshold)) return false;
@@ -114,10 +121,10 @@ struct Wf {
         const uint32_t u = (uint32_t)(g & kNull);
         if (u == kNull) { have = true; break; }
         help_phase2<kDeq>(r, u, c, me);
-        if (cas_acq_rel(G, g, (c << S) | kNull) == g) { have = true; break; }
+        if (cas_relaxed(G, g, (c << S) | kNull) == g) { have = true; break; }
       }
       const uint64_t want = local_word(c, tag) | kINC;      // L258: synchronize L to c using INC
-      if (!have || cas_acq_rel(L, v, want) != v) {
+      if (!have || cas_relaxed(L, v, want) != v) {
         v = ld_acquire(L);
         if (tag_of(v) != tag || (v & kFIN)) return false;
         if (!(v & kINC)) return true;                       // round already completed by another helper
@@ -132,15 +139,15 @@ struct Wf {
       st_relaxed(&mine->p2_target, target_id);
       st_relaxed(&mine->p2_expect, v);
       st_release(&mine->p2_seq2, s);
-      fence_acq_rel();
       const uint64_t g0 = (c << S) | kNull;
-      if (cas_acq_rel(G, g0, ((c + 1) << S) | me) == g0) break;        // L262: <c,NULL> -> <c+1,tid>
+      if (cas_acq_rel(G, g0, ((c + 1) << S) | me) == g0) break;        // L262: <c,NULL> -> <c+1,tid>; release: the record is visible to whoever reads this ThrIdx
+      bo.pause();                                                      // lost the round: thousands of losers must not keep G busy
     }
     ++(kDeq ? mine->n_head_inc : mine->n_tail_inc);
     if (kDeq) faa_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)-1ll);   // L264-266
     GQ_L_EVENT(r, target_id, 'W', me, v, c);
-    if (cas_acq_rel(L, v, v & ~kINC) == v) ++(kDeq ? mine->n_head_clr : mine->n_tail_clr);   // L270: clear INC on L
-    cas_acq_rel(G, ((c + 1) << S) | me, ((c + 1) << S) | kNull);         // L273: clear ThrIdx in G
+    if (cas_relaxed(L, v, v & ~kINC) == v) ++(kDeq ? mine->n_head_clr : mine->n_tail_clr);   // L270: clear INC on L
+    cas_relaxed(G, ((c + 1) << S) | me, ((c + 1) << S) | kNull);         // L273: clear ThrIdx in G
     v &= ~kINC;
     return true;
   }
@@ -161,7 +168,7 @@ struct Wf {
       uint64_t* L = &rec(r, tid)->localTail;
       const uint64_t v = ld_acquire(L);
       if ((v >> S) != h) return false;
-      if (!(v & 3)) cas_acq_rel(L, v, v | kFIN);
+      if (!(v & 3)) cas_relaxed(L, v, v | kFIN);
       return true;
     }
   };
@@ -179,22 +186,22 @@ struct Wf {
       if (cycle_newer<16>(c, F::cycle(E)) && cycle_newer<16>(c, F::note(E))) {
         const bool usable = F::vacant(E) && (F::safe(E) || R::counter(ld_acquire(r.head)) <= T);
         if (!usable) {                                        // Lemma III.8: advance Note, skip this slot
-          if (cas_acq_rel(sp, E, F::with_note(E, c)) != E) continue;
+          if (cas_relaxed(sp, E, F::with_note(E, c)) != E) continue;
           return false;
         }
         st_relaxed(r.owner + j, ((uint64_t)c << 32) | owner);
         const uint64_t N = F::installed_slow(E, c, x);        // <c, Safe 1, Enq 0, x>: linearization point
-        if (cas_acq_rel(sp, E, N) != E) continue;
+        if (cas_release(sp, E, N) != E) continue;          // release: Data[x] (ordered by the record's acquire) goes with the entry
         GQ_IDX_EVENT(3, r, x, T, E, v);
-        if (GQ_MUT(MUT_SLOW_NO_FIN) && (T & 3) == 0) { cas_acq_rel(sp, N, N | F::kEnqBit); return false; }
-        if (cas_acq_rel(L, v, v | kFIN) == v)                 // finalise the request ...
-          cas_acq_rel(sp, N, N | F::kEnqBit);                 // ... and make the entry visible to fast dequeuers
+        if (GQ_MUT(MUT_SLOW_NO_FIN) && (T & 3) == 0) { cas_relaxed(sp, N, N | F::kEnqBit); return false; }
+        if (cas_relaxed(L, v, v | kFIN) == v)                 // finalise the request ...
+          cas_relaxed(sp, N, N | F::kEnqBit);                 // ... and make the entry visible to fast dequeuers
         R::reset_threshold(r);
         return true;
       }
       if (F::cycle(E) == c && !F::vacant(E)) {                // installed by another helper of this request
         GQ_IDX_EVENT(4, r, x, T, E, v);
-        if (cas_acq_rel(L, v, v | kFIN) == v) cas_acq_rel(sp, E, E | F::kEnqBit);
+        if (cas_relaxed(L, v, v | kFIN) == v) cas_relaxed(sp, E, E | F::kEnqBit);
         R::reset_threshold(r);
         return true;
       }
@@ -204,7 +211,7 @@ struct Wf {
 
   // FIN on <H, tag>: true iff the request now is finished AT this ticket.
   __device__ __forceinline__ static bool set_fin(uint64_t* L, uint64_t v) {
-    const uint64_t o = cas_acq_rel(L, v, v | kFIN);
+    const uint64_t o = cas_relaxed(L, v, v | kFIN);
     return o == v || o == (v | kFIN);
   }
 
@@ -224,14 +231,14 @@ struct Wf {
       if (!F::vacant(E)) {                                    // occupied by another cycle's element
         if (cycle_newer<16>(c, F::cycle(E)) && cycle_newer<16>(c, F::note(E))) {
           const uint64_t En = F::with_note(E, c);             // later helpers make the same decision
-          if (cas_acq_rel(sp, E, En) != E) continue;
+          if (cas_relaxed(sp, E, En) != E) continue;
           E = En;
         }
         New = F::unsafe(E);
       } else {
         New = F::advanced(E, c);
       }
-      if (cycle_newer<16>(c, F::cycle(E)) && New != E && cas_acq_rel(sp, E, New) != E) continue;
+      if (cycle_newer<16>(c, F::cycle(E)) && New != E && cas_relaxed(sp, E, New) != E) continue;
       const uint64_t T = R::counter(ld_acquire(r.tail));
       if (T <= H + 1) {
         R::catchup_tail(r, H + 1);
