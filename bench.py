@@ -155,14 +155,14 @@ def run_apps(gq, torch, scale, fast_oracle=True):
     from paper_2606_01693_b200 import inputs
     out = {}
     t0 = time.perf_counter()
-    rowptr, col, src = inputs.rmat_csr(scale, 16, seed=1)
+    d_rowptr, d_col, src = inputs.rmat_csr_torch(scale, 16, seed=1, device="cuda")   # same arrays as inputs.rmat_csr (tests/test_inputs.py)
+    torch.cuda.synchronize()
     gen_s = time.perf_counter() - t0
+    rowptr, col = d_rowptr.cpu().numpy().astype(np.uint64), d_col.cpu().numpy().view(np.uint32)
     nv = len(rowptr) - 1
     t0 = time.perf_counter()
     ref, ref_edges = oracle.bfs(rowptr, col, src)
     cpu_s = time.perf_counter() - t0
-    d_rowptr = torch.from_numpy(rowptr.view(np.int64)).cuda()
-    d_col = torch.from_numpy(col.view(np.int32)).cuda()
     d_dist = torch.empty(nv, dtype=torch.int32, device="cuda")
     bfs = {"graph": f"R-MAT scale {scale}, edge factor 16, {nv} vertices, {len(col)} directed edges, source {src}",
            "generate_s": round(gen_s, 1),

@@ -212,7 +212,7 @@ int bfs_run_t(const uint64_t* d_rowptr, const uint32_t* d_col, uint32_t nv, uint
   gq_opts qo{};
   qo.max_threads = threads;
   qo.flags = o.flags | GQ_F_NO_DEQ_SPIN | GQ_F_EAGER_EMPTY | GQ_F_NO_FULL_TEST;   // each vertex is enqueued at most once: never nv items;   // nothing arrives in `cur` during a level: never park
-  qo.ymc_pool_cells = 2ull * nv + 64ull * threads + (1u << 16);
+  qo.ymc_pool_cells = 0;                                  // G-WFQ-YMC: the default ring pool, pow2ceil(capacity + 4k) cells (Y10)
   OwnedQueue<Q> qa, qb;
   const uint64_t cap = pow2ceil64(std::max<uint32_t>(nv, 2));
   int rc = qa.create(cap, qo);
@@ -538,7 +538,7 @@ int rt_render_t(const gq_rt_scene& sc, float* d_rgb, gq_rt_stats* st_out, cudaSt
   qo.max_threads = threads;
   qo.park_ns = 20000;                                     // a warp waits on its slot only for an item whose enqueuer is in flight
   qo.flags = GQ_F_EAGER_EMPTY | GQ_F_NO_FULL_TEST;        // idle warps poll: EMPTY at once when Tail <= Head; never more than n_items items
-  qo.ymc_pool_cells = 4ull * a.n_items * (sc.max_bounce + 2) + 64ull * threads + (1u << 16);
+  qo.ymc_pool_cells = 0;                                  // G-WFQ-YMC: the default ring pool, pow2ceil(capacity + 4k) cells, stays L2-resident (Y10)
   OwnedQueue<Q> q;
   int rc = q.create(pow2ceil64(std::max<uint32_t>(a.n_items, 2)), qo);
   if (rc) return rc;
