@@ -56,7 +56,6 @@ enum : uint32_t { LAT_HEAD_FAA = 0, LAT_SLOT_WAIT = 1, LAT_TAIL_FAA = 2, LAT_INS
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
 struct LfqFmt {
-  static constexpr bool kAcquireSlot = false;            // see try_deq L176
   static constexpr int kCycBits = 31;
   static constexpr int kCtrShift = 0;                    // Head/Tail are plain counters
   static constexpr uint32_t kBotC = 0xFFFFFFFFu;         // consumed   (reading G3)
@@ -87,7 +86,6 @@ struct LfqFmt {
 //      index, and vacancy is a bit of its own so that every 32-bit value can be stored:
 //      [63:34] Cycle(30) | [33] Safe | [32] Vacant | [31:0] payload
 struct DirFmt {
-  static constexpr bool kAcquireSlot = false;
   static constexpr int kCycBits = 30;
   static constexpr int kCtrShift = 0;
   static constexpr uint32_t kBotC = 0xFFFFFFFFu;
@@ -113,7 +111,6 @@ struct DirFmt {
 // ---- G-WFQ entry word (Fig. 2 missing -> reading W1):
 //      [63:48] Cycle(16) | [47:32] Note(16) | [31] Safe | [30] Enq | [29:0] Index(30)
 struct WfqFmt {
-  static constexpr bool kAcquireSlot = true;             // slow-path installs hand their payload over by release / acquire
   static constexpr int kCycBits = 16;
   static constexpr int kCtrShift = 20;                   // Head/Tail word: counter(44) | ThrIdx(20)
   static constexpr uint32_t kBotC = 0x3FFFFFFFu;
@@ -351,9 +348,10 @@ struct Ring {
     uint32_t waited = 0, nap = 0;
     GQ_TIC(t1);
     for (;;) {
-      // L176.  Acquire where the entry publishes something else (fenced payload, G-WFQ's slow-path installs: G15); with
-      // the tagged payload cell (D6) or the payload in the entry itself nothing hangs on this load: relaxed, no CCTL.IVALL per poll
-      uint64_t E = (F::kAcquireSlot || (flags & kFencedPayload)) ? ld_acquire(sp) : ld_relaxed(sp);
+      // L176.  Acquire in every build: it is the consumer side of the hand-over contract of queue.cuh (reading G15): what a
+      // producer wrote before __threadfence(); enqueue(v) is visible to the thread that dequeued v.  (A relaxed poll where the
+      // library itself needs no edge, D6 / direct payload, was tried: +0.4 %, and the user-kernel litmus failed at once.)
+      uint64_t E = ld_acquire(sp);
     classify:
       if (F::cycle(E) == c && !F::vacant(E)) {                        // L178
         GQ_TOC(LAT_SLOT_WAIT + 5 * r.id, t1, E);
