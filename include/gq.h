@@ -109,6 +109,13 @@ int queue_reset    (gq_queue* q, void* stream);
 int queue_prefill  (gq_queue* q, const uint32_t* host_vals, uint64_t count, void* stream);
 /* Dequeue until EMPTY or `max` items, in FIFO order, into host_out (HOST). */
 int queue_drain    (gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream);
+/* queue_drain for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+   cudaMalloc): same arguments, same result, but the staging memory is a static device array inside the library instead of
+   two cudaMalloc'ed blocks; the call makes no cudaMalloc / cudaFree.  max > GQ_DRAIN_NOALLOC_MAX returns GQ_E_INVAL with a
+   message in gq_last_cuda_error() (drain in pieces, or use queue_drain).  All calls on one GPU share that array: calls that
+   overlap on the GPU (two host threads, two streams) race. */
+#define GQ_DRAIN_NOALLOC_MAX 65536u
+int queue_drain_noalloc(gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream);
 /* Copy the POD device view (gq::LfqView / WfqView / YmcView of include/gq/queue.cuh) that user
    kernels take by value.  view_out: HOST, view_bytes must be >= sizeof(view). */
 int queue_device_view(const gq_queue* q, void* view_out, size_t view_bytes);

@@ -39,7 +39,7 @@ class GqError(RuntimeError):
             if os.environ.get("GQ_EXIT_ON_TIMEOUT"):      # test runs: every later CUDA call (frees included) would block on the stuck kernel
                 os.write(2, f"\n[gq] {where}: watchdog time-out, kernel still running; exiting (GQ_EXIT_ON_TIMEOUT)\n".encode())
                 os._exit(3)
-        detail = lib.gq_last_cuda_error().decode() if code in (GQ_E_CUDA, GQ_E_TIMEOUT, GQ_E_NOMEM) else ""
+        detail = lib.gq_last_cuda_error().decode() if code in (GQ_E_CUDA, GQ_E_TIMEOUT, GQ_E_NOMEM) or where == "queue_drain_noalloc" else ""
         super().__init__(f"{where}: GQ_E_{_ERR.get(code, code)} {detail}".strip())
 
 
@@ -98,7 +98,7 @@ HIST_DTYPE = np.dtype([("proc", "<u4"), ("op", "<u4"), ("arg", "<u4"), ("ret_sta
 
 # every symbol include/gq.h declares
 SYMBOLS = ("queue_storage_bytes", "queue_create", "queue_create_ex", "queue_destroy", "queue_reset", "queue_prefill",
-           "queue_drain", "queue_device_view", "queue_kind", "queue_max_coresident_threads", "run_balanced",
+           "queue_drain", "queue_drain_noalloc", "queue_device_view", "queue_kind", "queue_max_coresident_threads", "run_balanced",
            "run_split", "run_faa_ceiling", "run_slot_atomic_ceiling", "run_warp_faa_probe", "run_funnel_probe", "queue_run_script",
            "history_dump", "bfs_run", "bfs_run_ex", "rt_render", "rt_render_ex", "gq_last_cuda_error", "gq_version",
            "gq_dbg_sites", "gq_dbg_trace", "gq_set_mutation", "queue_debug_counters")
@@ -116,6 +116,7 @@ def _load(variant=""):
     L.queue_reset.argtypes = [C.c_void_p, C.c_void_p]
     L.queue_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     L.queue_drain.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(C.c_uint64), C.c_void_p]
+    L.queue_drain_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(C.c_uint64), C.c_void_p]
     L.queue_device_view.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
     L.queue_kind.argtypes = [C.c_void_p]
     L.queue_debug_counters.argtypes = [C.c_void_p, C.c_void_p]
@@ -198,6 +199,17 @@ def queue_drain(q, max_items, stream=None):
     out = np.empty(max(int(max_items), 1), np.uint32)
     n = C.c_uint64(0)
     _chk(lib.queue_drain(q, _np_ptr(out), int(max_items), C.byref(n), stream), "queue_drain")
+    return out[: n.value].copy()
+
+
+GQ_DRAIN_NOALLOC_MAX = 65536
+
+
+def queue_drain_noalloc(q, max_items, stream=None):
+    """queue_drain without any device allocation (static scratch inside the library); max_items <= GQ_DRAIN_NOALLOC_MAX."""
+    out = np.empty(max(int(max_items), 1), np.uint32)
+    n = C.c_uint64(0)
+    _chk(lib.queue_drain_noalloc(q, _np_ptr(out), int(max_items), C.byref(n), stream), "queue_drain_noalloc")
     return out[: n.value].copy()
 
 

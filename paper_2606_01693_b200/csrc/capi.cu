@@ -880,6 +880,58 @@ extern "C" int queue_drain(gq_queue* q, uint32_t* host_out, uint64_t max, uint64
   return dispatch(q, [&](auto& view) { return drain_t(view, host_out, max, n_out, st, lanes); });
 }
 
+// ---- queue_drain_noalloc: the same drain for callers that must not allocate (gq.h) ------------------------------------
+// The staging memory of queue_drain (item count + items) in a file-scope device array instead of two cudaMalloc'ed blocks.
+// Every device that loads libgq.so holds these 256 B + 256 KiB until the process exits.  In HOST code the name
+// g_drain_scratch is a host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress, once per
+// device, with that device current.  All calls share the array (it keeps the last call's contents; the count word is
+// cleared before each launch): calls that overlap on one GPU race.
+static __device__ __align__(256) unsigned char g_drain_scratch[256 + (size_t)GQ_DRAIN_NOALLOC_MAX * 4];
+static int drain_scratch_address(unsigned char** out) {
+  constexpr int kMaxDevices = 64;
+  static unsigned char* addr[kMaxDevices] = {};
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) { gq_set_error("queue_drain_noalloc: device index beyond 63"); return GQ_E_INVAL; }
+  if (!addr[dev]) {
+    void* p = nullptr;
+    CU(cudaGetSymbolAddress(&p, g_drain_scratch));       // resolves against the current device
+    addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = addr[dev];
+  return 0;
+}
+template <class Q>
+static int drain_noalloc_t(const Q& view, unsigned char* scratch, uint32_t* host_out, uint64_t max, uint64_t* n_out, cudaStream_t st, uint32_t lanes) {
+  uint64_t* d_n = reinterpret_cast<uint64_t*>(scratch);
+  uint32_t* d_out = reinterpret_cast<uint32_t*>(scratch + 256);
+  uint64_t n = 0;
+  CU(cudaMemsetAsync(d_n, 0, 8, st));                    // the array keeps the last call's contents
+  drain_kernel<Q><<<1, 32, 0, st>>>(view, d_out, max, d_n, lanes);
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(&n, d_n, 8, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  if (n > max) { gq_set_error("queue_drain_noalloc: count beyond max"); return GQ_E_STATE; }
+  if (n) CU(cudaMemcpy(host_out, d_out, n * 4, cudaMemcpyDeviceToHost));
+  *n_out = n;
+  return 0;
+}
+extern "C" int queue_drain_noalloc(gq_queue* q, uint32_t* host_out, uint64_t max, uint64_t* n_out, void* stream) {
+  if (!q || !n_out || (!host_out && max)) return GQ_E_INVAL;
+  if (max > GQ_DRAIN_NOALLOC_MAX) {
+    std::snprintf(g_err, sizeof g_err, "queue_drain_noalloc: max = %llu items exceeds GQ_DRAIN_NOALLOC_MAX = %u (static scratch); drain in pieces or use queue_drain",
+                  (unsigned long long)max, (unsigned)GQ_DRAIN_NOALLOC_MAX);
+    return GQ_E_INVAL;
+  }
+  unsigned char* scratch = nullptr;
+  int rc = drain_scratch_address(&scratch);
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  q->fresh = false;
+  const uint32_t lanes = std::min(32u, q->max_threads);
+  return dispatch(q, [&](auto& view) { return drain_noalloc_t(view, scratch, host_out, max, n_out, st, lanes); });
+}
+
 template <class Q>
 static int script_t(const Q& view, const uint32_t* op, const uint32_t* arg, uint64_t count, uint32_t tid, uint32_t* st_out, uint32_t* val_out) {
   uint32_t* d = nullptr;
