@@ -342,7 +342,7 @@ def run_ours(args, rank, world, local_rank):
         qs = gq.queue_create_ex(kind, 1 << 20, gq.gq_opts(ymc_pool_cells=YMC_POOL_CELLS))
         pre = np.arange(1 << 19, dtype=np.uint32)
         runs = {}
-        for layout in (0, 1):
+        for layout in (0, 1, 2):
             xs = []
             for _ in range(3):
                 gq.queue_reset(qs)
@@ -357,7 +357,13 @@ def run_ours(args, rank, world, local_rank):
                           "workload": "BJ#3 split, p = 0.5, capacity 2^20 prefilled 2^19, seeded Bernoulli roles (mixed warps), median of 3 x 100 ms",
                           "runs_gops": [round(x / 1e9, 2) for x in runs[0]],
                           "same_roles_on_homogeneous_warps_gops": [round(x / 1e9, 2) for x in runs[1]],
-                          "note": "mixed warps: every WAVEFAA batch holds about 16 tickets instead of 32 (DESIGN.md section 7)"}
+                          "mixed_warps_fused_step_gops": [round(x / 1e9, 2) for x in runs[2]],
+                          "peak_mixed_warps": c1_tps / 1e9,
+                          "frac_of_mixed_peak": a0 / c1_tps,
+                          "note": "mixed warps: every WAVEFAA batch holds about 16 tickets instead of 32, so an operation costs the hot "
+                                  "counters twice the atomics: their capacity allows 2 x C1 x 16/32 = C1 (peak_mixed_warps).  "
+                                  "mixed_warps_fused_step_gops: the same roles through gq::enqueue_or_dequeue_step "
+                                  "(gq_run_cfg.role_layout = 2, DESIGN.md D12)"}
     except gq.GqError as e:
         roofline_split = {"error": str(e)}
 

@@ -149,10 +149,13 @@ typedef struct {
                                   1 = same seeded roles, but the logical threads are placed so that producers fill the
                                   first physical threads and consumers the rest: warps are homogeneous (at most one mixed);
                                   2 = layout 0, but each iteration is ONE converged call of the fused operation
-                                  gq::enqueue_or_dequeue (G-LFQ only): the two roles of a mixed warp overlap */
+                                  gq::enqueue_or_dequeue_step (G-LFQ only): the two roles of a mixed warp overlap, and a
+                                  lane that has to wait in line hands the wait back instead of holding up its warp (D12);
+                                  4 = the same with the blocking gq::enqueue_or_dequeue; 3 = layout 1 through the fused
+                                  operation (diagnostic: homogeneous warps, one address group) */
   uint32_t converged;          /* 1: the lanes of a warp start every iteration of the benchmark loop together (one ballot per
                                   iteration), as a lock-step wavefront would; 0: a lane starts its next operation as soon as its
-                                  last one returns.  Balanced and split loops; not the fused role_layout 2 */
+                                  last one returns */
   uint32_t block_faa;          /* 1: the warps of a block combine their ticket requests per hot counter in shared memory: one global
                                   FAA per batch instead of one per warp (block-level funnel, D11; include/gq/queue.cuh) */
   uint32_t funnel_window_ns;   /* block_faa: a batch stays open this long so that more warps can join (0 = closed at once) */

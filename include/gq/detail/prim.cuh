@@ -11,6 +11,7 @@
 // WAVEFAA (Alg. 1, Lemma III.1) is warp_faa() below, re-derived for
 // 32-lane warps with independent thread scheduling (reading G10).
 #pragma once
+#include <climits>
 #include <cstdint>
 #include <cstdio>
 
@@ -187,8 +188,9 @@ __device__ __forceinline__ uint64_t funnel_faa(BlockFunnel* f, uint64_t* counter
 
 template <bool kUniform>
 __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 1, BlockFunnel* funnel = nullptr) {
-  uint32_t mask = __activemask();
-  if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
+  const uint32_t active = __activemask();
+  uint32_t mask = active;
+  if (!kUniform) mask = __match_any_sync(active, reinterpret_cast<unsigned long long>(counter));
 #ifdef GQ_DBG_SITES
   if (kUniform && __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter)) != mask) GQ_COUNT(71, 1);   // kUniform promise broken
 #endif
@@ -203,9 +205,14 @@ __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 
     base = faa_relaxed(counter, (uint64_t)__popc(mask) * unit);
 #ifdef GQ_DBG_SITES
     if ((blockIdx.x & 63u) == 0) { GQ_COUNT(20, 1); GQ_COUNT(21, __popc(mask)); }   // WAVEFAA batch size (sampled blocks)
+    if ((blockIdx.x & 63u) == 0 && lane_id() == (uint32_t)__ffs(active) - 1) { GQ_COUNT(24, 1); GQ_COUNT(25, __popc(active)); }   // converged set
 #endif
   }
-  base = __shfl_sync(mask, base, leader);
+  // One shuffle over the converged set, every lane reading from the leader of its own group.  (A shuffle per group,
+  // __shfl_sync(mask, ..), is a WARPSYNC on lane-dependent masks: measured on sm_100a, it splits the converged warp
+  // into its address groups for good, and the groups then run one after the other, each waiting out the other's L2
+  // round trips: the fused mixed-role operation of lfq.cuh was no faster than two diverged calls because of it.)
+  base = __shfl_sync(active, base, leader);
   return base + (uint64_t)rank * unit;
 }
 // Two WAVEFAAs issued back to back by the same leader before either result is consumed: the two
@@ -213,10 +220,11 @@ __device__ __forceinline__ uint64_t warp_faa(uint64_t* counter, uint64_t unit = 
 // each counter separately: one group, one leader, one FAA per counter, ranks from the same mask.
 template <bool kUniform>
 __device__ __forceinline__ void warp_faa2(uint64_t* ca, uint64_t* cb, uint64_t unit_a, uint64_t unit_b, uint64_t* a, uint64_t* b) {
-  uint32_t mask = __activemask();
+  const uint32_t active = __activemask();
+  uint32_t mask = active;
   if (!kUniform) {
-    const uint32_t ma = __match_any_sync(mask, reinterpret_cast<unsigned long long>(ca));
-    mask = ma & __match_any_sync(mask, reinterpret_cast<unsigned long long>(cb));
+    const uint32_t ma = __match_any_sync(active, reinterpret_cast<unsigned long long>(ca));
+    mask = ma & __match_any_sync(active, reinterpret_cast<unsigned long long>(cb));
   }
   const uint32_t leader = __ffs(mask) - 1;
   const uint32_t rank = __popc(mask & lanemask_lt());
@@ -225,8 +233,8 @@ __device__ __forceinline__ void warp_faa2(uint64_t* ca, uint64_t* cb, uint64_t u
     ba = faa_relaxed(ca, (uint64_t)__popc(mask) * unit_a);
     bb = faa_relaxed(cb, (uint64_t)__popc(mask) * unit_b);
   }
-  ba = __shfl_sync(mask, ba, leader);
-  bb = __shfl_sync(mask, bb, leader);
+  ba = __shfl_sync(active, ba, leader);
+  bb = __shfl_sync(active, bb, leader);
   *a = ba + (uint64_t)rank * unit_a;
   *b = bb + (uint64_t)rank * unit_b;
 }
@@ -244,13 +252,14 @@ __device__ __forceinline__ uint64_t lane_faa(uint64_t* counter, uint64_t unit = 
 // a lane-ordered sequence of single decrements would have returned.
 template <bool kUniform>
 __device__ __forceinline__ int64_t warp_dec(int64_t* counter) {
-  uint32_t mask = __activemask();
-  if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(counter));
+  const uint32_t active = __activemask();
+  uint32_t mask = active;
+  if (!kUniform) mask = __match_any_sync(active, reinterpret_cast<unsigned long long>(counter));
   const uint32_t leader = __ffs(mask) - 1;
   const uint32_t rank = __popc(mask & lanemask_lt());
   uint64_t base = 0;
   if (lane_id() == leader) base = faa_relaxed(reinterpret_cast<uint64_t*>(counter), (uint64_t)(-(int64_t)__popc(mask)));
-  base = __shfl_sync(mask, base, leader);
+  base = __shfl_sync(active, base, leader);
   return (int64_t)base - (int64_t)rank;
 }
 

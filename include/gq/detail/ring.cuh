@@ -38,7 +38,16 @@ struct RingView {
 
 namespace detail {
 
-enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2 };
+enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2, RING_PENDING = 3 };
+// A dequeue attempt that waits in line (D2) without blocking its caller: try_deq hands the wait back (RING_PENDING) with the
+// ticket it holds, and the caller comes back later with the same record; the parking budget is then counted in looks at the
+// slot, `step_ns` each.  The holder of a ticket MUST come back until the attempt ends otherwise: the enqueuer that draws the
+// same ticket will install an item for it.
+struct DeqWait {
+  uint64_t ticket = 0;
+  uint32_t waited = 0;     // ns of the parking budget used so far; 0 = no attempt pending
+  uint32_t step_ns = 2048; // what one round of the caller's loop is charged
+};
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
 enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
                   kThrFirst = 32u, kNoPairedFaa = 64u, kThrRedMax = 128u, kFencedPayload = 256u, kEagerEmpty = 512u, kNoCellPrefetch = 1024u, kNoFullTest = 2048u,
@@ -52,7 +61,8 @@ enum : uint32_t { SITE_ENQ_CAS_LOST = 0, SITE_ENQ_UNSAFE = 1, SITE_ENQ_SLOT_AHEA
                   SITE_DEQ_EMPTY_THR = 12, SITE_DEQ_EMPTY_EARLY = 13, SITE_DEQ_EMPTY_PROBE = 14, SITE_DEQ_REPAIR = 15 };
 // latency probe sites (GQ_TIC / GQ_TOC): + 5 * ring id for the first five
 enum : uint32_t { LAT_HEAD_FAA = 0, LAT_SLOT_WAIT = 1, LAT_TAIL_FAA = 2, LAT_INSTALL_CAS = 3, LAT_THR_CHECK = 4,
-                  LAT_PAYLOAD = 10, LAT_ENQUEUE = 11, LAT_DEQUEUE = 12 };
+                  LAT_PAYLOAD = 10, LAT_ENQUEUE = 11, LAT_DEQUEUE = 12,
+                  LAT_STEP_PENDING_ENQ = 13, LAT_STEP_PENDING_DEQ = 14 /* enqueue_or_dequeue_step calls that handed the wait back */ };
 
 // ---- G-LFQ entry word (Alg. 1 <c,1,x>):  [63:33] Cycle(31) | [32] Safe | [31:0] Index
 struct LfqFmt {
@@ -212,11 +222,23 @@ struct Ring {
   // converged lanes agree on their largest target and only the leader touches the hot word
   // (one atomic per warp instead of 32 on the same address).
   __device__ __forceinline__ static void catchup_tail(const RingView& r, uint64_t target) {
-    uint32_t mask = __activemask();
-    if (!kUniform) mask = __match_any_sync(mask, reinterpret_cast<unsigned long long>(r.tail));
+    const uint32_t active = __activemask();
+    uint32_t mask = active;
+    if (!kUniform) mask = __match_any_sync(active, reinterpret_cast<unsigned long long>(r.tail));
     const uint32_t leader = __ffs(mask) - 1;
-    const uint64_t base = __shfl_sync(mask, target, leader);
-    const int dmax = __reduce_max_sync(mask, (int)(int64_t)(target - base));   // tickets of one warp are close
+    const uint64_t base = __shfl_sync(active, target, leader);         // over the converged set, see warp_faa
+    const int d = (int)(int64_t)(target - base);                        // tickets of one warp are close
+    int dmax = d;
+    if (kUniform) {
+      dmax = __reduce_max_sync(active, d);
+    } else {                                                            // one converged reduction per address group
+      for (uint32_t rest = active; rest;) {
+        const uint32_t g = __shfl_sync(active, mask, __ffs(rest) - 1);
+        const int m = __reduce_max_sync(active, mask == g ? d : INT_MIN);
+        if (mask == g) dmax = m;
+        rest &= ~g;
+      }
+    }
     if (lane_id() != leader) return;
     target = base + (int64_t)dmax;
     if (F::kCtrShift == 0) {
@@ -315,15 +337,20 @@ struct Ring {
   //     test is then made with the ticket in the place of Head, and parking (D2) is skipped when it
   //     says "empty" or Threshold was negative, which leaves the listing's own steps.  kThrFirst
   //     restores the listed order.
+  //  nb != nullptr: non-blocking parking (DeqWait above).  nb->waited != 0 resumes the attempt that holds nb->ticket.
   template <class Finalize>
   __device__ __forceinline__ static int try_deq(const RingView& r, uint32_t* x, uint64_t* h_out, const Finalize& fin,
-                                                bool probe = false, uint32_t flags = 0) {
+                                                bool probe = false, uint32_t flags = 0, DeqWait* nb = nullptr) {
     uint32_t park_ns = (flags & kNoDeqSpin) ? 0u : r.park_ns;
     int64_t thr;
     uint64_t h;
     const bool listed = probe || (flags & kThrFirst);
+    const bool resume = nb && nb->waited != 0;
     GQ_TIC(t0);
-    if (listed) {
+    if (resume) {
+      h = nb->ticket;                                                  // drawn by the call that returned RING_PENDING
+      thr = r.thr_reset;
+    } else if (listed) {
       thr = (int64_t)ld_relaxed(reinterpret_cast<const uint64_t*>(r.threshold));
       if (thr < 0) { GQ_SITE(SITE_DEQ_EMPTY_EARLY); return RING_EMPTY; }   // L166-169
       if (!(flags & kNoProbe) && (probe || thr != r.thr_reset)) {     // D1
@@ -345,7 +372,7 @@ struct Ring {
     uint64_t* sp = slot(r, j);
     // park budget in ns: every look at the slot counts its nap plus kPollNs (an L2 round trip under load)
     constexpr uint32_t kPollNs = 384;
-    uint32_t waited = 0, nap = 0;
+    uint32_t waited = resume ? nb->waited : 0u, nap = 0;
     GQ_TIC(t1);
     for (;;) {
       // L176.  Acquire in every build: it is the consumer side of the hand-over contract of queue.cuh (reading G15): what a
@@ -397,6 +424,11 @@ struct Ring {
           //  threads must stay off the hot lines, which is the point of D2.)
           // The first spin_ns are pure re-reading (the front of the line: the hand-over is detected one nap
           // earlier), after that the nap ladder 32 ns .. park_nap keeps the many threads further back quiet.
+          if (nb) {                                                    // wait handed back to the caller, ticket kept
+            nb->ticket = h;
+            nb->waited = waited + nb->step_ns;
+            return RING_PENDING;
+          }
           if (waited >= r.spin_ns && r.park_nap) { nap = nap ? (nap * 2 < r.park_nap ? nap * 2 : r.park_nap) : 32; __nanosleep(nap); }
           waited += nap + kPollNs;
           continue;

@@ -219,4 +219,70 @@ __device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& 
   }
 }
 
+// The same fused operation with the wait handed back to the caller (D12).  enqueue_or_dequeue keeps a converged
+// warp together, but a lane that has to wait in line (an enqueuer for a free index when the queue is full, a dequeuer for an
+// item when it is empty: D2) then holds up the 31 others, and at p = 0.5 BASELINE.json's split benchmark sits at one of the
+// two boundaries for most of its run.  Here a lane whose slot is still vacant returns PENDING at once, keeps its ticket in
+// `st`, and looks at the slot again on its next call, while the other lanes of the warp complete whole operations: one
+// converged chain of L2 round trips per call whatever the number of lanes that wait.
+// Contract: after PENDING the thread must call again with the same `st`, role and *v until it gets another result (it holds
+// a ticket; the enqueuer of that ticket will install an entry for it).  The operation's interval in a history runs from
+// its first call to the call that completes it.  The parking budget (gq_opts.park_ns) is charged st.step_ns per call.
+using op_state = detail::DeqWait;
+enum : int { PENDING = 3 };
+template <int kWarpFaa = true>
+__device__ __forceinline__ int enqueue_or_dequeue_step(const LfqView& q, thread_ctx& ctx, op_state& st, bool is_enq, uint32_t* v,
+                                                       uint64_t* retries = nullptr) {
+  using namespace detail;
+  using R = Ring<LfqFmt, false, kWarpFaa>;
+  uint64_t dummy = 0; if (!retries) retries = &dummy;
+  if (q.flags & kFencedPayload) return is_enq ? enqueue<false, kWarpFaa>(q, ctx, *v, retries) : dequeue<false, kWarpFaa>(q, ctx, v, retries);
+  RingView r1 = is_enq ? q.fq : q.aq, r2 = is_enq ? q.aq : q.fq;        // per-lane ring pair
+  const uint32_t hbit = is_enq ? 2u : 1u;
+  uint32_t idx = 0;
+  uint64_t h1 = 0;
+  int s;
+  GQ_TIC(t_op);
+  {
+    Backoff bo;
+    [[maybe_unused]] uint32_t sn = 0;
+    bool probe = (ctx.hungry & hbit) != 0;
+    for (;;) {
+      if (GQ_STUCK(sn, 6, ctx.tid, r1.head, r1.tail)) { s = RING_EMPTY; break; }
+      s = R::try_deq(r1, &idx, &h1, NoFinalize{}, probe, q.flags, &st);
+      if (s != RING_RETRY) break;
+      st.waited = 0;                                                   // that ticket is spent: next attempt draws a new one
+      ++*retries;
+      probe = true;
+      bo.pause();
+    }
+  }
+  if (s == RING_PENDING) { GQ_TOC(is_enq ? LAT_STEP_PENDING_ENQ : LAT_STEP_PENDING_DEQ, t_op, h1); return PENDING; }
+  st.waited = 0;
+  if (s == RING_EMPTY) {
+    ctx.hungry |= hbit;
+    return is_enq ? FULL : EMPTY;
+  }
+  ctx.hungry &= ~hbit;
+  if (!is_enq) ctx.last_ticket = h1;
+  uint64_t* cell = q.data + idx;
+  uint64_t w = is_enq ? 0 : ld_relaxed(cell);
+  Backoff bo;
+  [[maybe_unused]] uint32_t sn = 0;
+  for (bool first = true;; first = false) {
+    if (GQ_STUCK(sn, 4, ctx.tid, r2.head, r2.tail)) return OK;
+    const uint64_t t = R::take(r2, false);                               // one leader per counter, one instruction
+    if (is_enq) {
+      st_relaxed(cell, cell_word(t, *v));                              // D6: payload tagged with its AQ ticket
+    } else if (first) {
+      w = cell_await(cell, w, h1);
+      *v = (uint32_t)w;
+    }
+    uint64_t tt;
+    if (R::try_enq(r2, idx, &tt, q.flags | kRelaxedInstall, true, t) == RING_OK) { GQ_TOC(is_enq ? LAT_ENQUEUE : LAT_DEQUEUE, t_op, tt); return OK; }
+    ++*retries;
+    bo.pause();
+  }
+}
+
 }  // namespace gq

@@ -659,7 +659,7 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   const bool hist = cfg->record_history != 0;
   if (hist && cfg->ops_per_thread == 0) return GQ_E_INVAL;
   if (!hist && cfg->ops_per_thread == 0 && cfg->duration_ms <= 0) return GQ_E_INVAL;
-  const bool fused = mode == MODE_SPLIT && cfg->role_layout == 2;       // mixed warps, one converged call (G-LFQ)
+  const bool fused = mode == MODE_SPLIT && cfg->role_layout >= 2 && cfg->role_layout <= 4;       // mixed warps, one converged call (G-LFQ)
   if (fused && (q->kind != GQ_LFQ || per_lane)) return GQ_E_INVAL;
   if (hist && per_lane) return GQ_E_INVAL;                              // the per-thread-FAA ablation is a timing variant only
   const bool funnel = cfg->block_faa != 0;                              // block-level ticket funnels (D11): a kernel variant of its own
@@ -691,7 +691,7 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
   Q v = view;
   set_nthreads(v, r.threads);          // help ring = the launched threads (reading W7)
   LaunchRes lr;
-  if (mode == MODE_SPLIT && cfg->role_layout == 1) {   // same seeded roles, producers first: homogeneous warps
+  if (mode == MODE_SPLIT && (cfg->role_layout == 1 || cfg->role_layout == 3)) {   // same seeded roles, producers first: homogeneous warps
     std::vector<uint32_t> perm; perm.reserve(r.threads);
     std::vector<uint32_t> cons; cons.reserve(r.threads);
     for (uint32_t t = 0; t < r.threads; ++t)
@@ -700,8 +700,9 @@ static int run_bench_t(gq_queue* q, const Q& view, const gq_run_cfg* cfg, int mo
     CU(cudaMalloc(&lr.scratch, (size_t)r.threads * 4));
     CU(cudaMemcpy(lr.scratch, perm.data(), (size_t)r.threads * 4, cudaMemcpyHostToDevice));
     p.perm = static_cast<const uint32_t*>(lr.scratch);
-  } else if (mode == MODE_SPLIT && cfg->role_layout == 2) {
-    p.fused = 1;
+    if (cfg->role_layout == 3) p.fused = 1;          // homogeneous warps through the fused operation (diagnostic)
+  } else if (mode == MODE_SPLIT && (cfg->role_layout == 2 || cfg->role_layout == 4)) {
+    p.fused = cfg->role_layout == 2 ? 1 : 2;           // 2: enqueue_or_dequeue_step (waits handed back), 4: the blocking enqueue_or_dequeue
   } else if (cfg->role_layout != 0 && mode == MODE_SPLIT) {
     return GQ_E_INVAL;
   }

@@ -41,6 +41,12 @@ template <int kWarpFaa>
 __device__ __forceinline__ int fused_op(const LfqView& q, thread_ctx& ctx, bool is_enq, uint32_t* v, uint64_t* retries) {
   return enqueue_or_dequeue<kWarpFaa>(q, ctx, is_enq, v, retries);
 }
+template <int kWarpFaa, class Q>
+__device__ __forceinline__ int fused_step(const Q&, thread_ctx&, op_state&, bool, uint32_t*, uint64_t*) { return -1; }
+template <int kWarpFaa>
+__device__ __forceinline__ int fused_step(const LfqView& q, thread_ctx& ctx, op_state& st, bool is_enq, uint32_t* v, uint64_t* retries) {
+  return enqueue_or_dequeue_step<kWarpFaa>(q, ctx, st, is_enq, v, retries);
+}
 
 __device__ __forceinline__ uint64_t warp_sum(uint64_t v) {
 #pragma unroll
@@ -142,23 +148,34 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
     const bool do_enq = !split || (uint64_t)mix32(p.seed * 0x9e3779b9u + ltid) < p.prod_threshold;
     gq_hist_rec* my = kHist ? hist + (size_t)ltid * p.ops_per_thread * (split ? 1 : 2) : nullptr;
     if (kFused && HasFused<Q>::value) {                     // split mode, mixed warps, one converged call per iteration
-      for (uint32_t iter = 0;; ++iter) {
+      // p.fused == 1: gq::enqueue_or_dequeue_step, lanes that have to wait in line hand the wait back (PENDING) and the warp
+      // goes on; the operation of such a lane spans several iterations.  p.fused == 2: the blocking gq::enqueue_or_dequeue.
+      uint32_t act = __activemask();
+      op_state st;
+      uint32_t iter = 0;
+      uint64_t t_call = 0;
+      for (;;) {
         uint32_t v = payload_of(p, ltid, iter);
         const uint32_t v_in = v;
-        uint64_t t_call = 0;
-        if (kHist) {
+        if (kHist && st.waited == 0) {
           if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
           t_call = globaltimer_ns();
         }
-        const int s = fused_op<kWarpFaa>(q, ctx, do_enq, &v, &a.retries);
+        const int s = p.fused == 2 ? fused_op<kWarpFaa>(q, ctx, do_enq, &v, &a.retries)
+                                   : fused_step<kWarpFaa>(q, ctx, st, do_enq, &v, &a.retries);
         if (kHist) { __threadfence(); }
         const uint64_t now = globaltimer_ns();
-        if (kHist) *my++ = do_enq ? gq_hist_rec{ltid, GQ_OP_ENQ, v_in, (uint32_t)s, 0u, 0u, t_call, now}
-                                  : gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
-        const bool in = now >= tw && now < te;
-        if (do_enq) { if (s == OK) { ++a.tot_enq; a.sum_enq += v_in; a.succ_enq += in; } else { ++a.tot_full; a.full += in; } }
-        else        { if (s == OK) { ++a.tot_deq; a.sum_deq += v; a.succ_deq += in; } else { ++a.tot_empty; a.empty += in; } }
-        if (fixed ? (iter + 1 >= p.ops_per_thread) : (now >= te)) break;
+        bool done = false;
+        if (s != PENDING) {
+          if (kHist) *my++ = do_enq ? gq_hist_rec{ltid, GQ_OP_ENQ, v_in, (uint32_t)s, 0u, 0u, t_call, now}
+                                    : gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
+          const bool in = now >= tw && now < te;
+          if (do_enq) { if (s == OK) { ++a.tot_enq; a.sum_enq += v_in; a.succ_enq += in; } else { ++a.tot_full; a.full += in; } }
+          else        { if (s == OK) { ++a.tot_deq; a.sum_deq += v; a.succ_deq += in; } else { ++a.tot_empty; a.empty += in; } }
+          ++iter;
+          done = fixed ? (iter >= p.ops_per_thread) : (now >= te);   // a pending operation is always brought to its end
+        }
+        if (loop_done(p, act, done)) break;
       }
     } else if (!split) {
       uint32_t act = __activemask();

@@ -500,10 +500,27 @@ def test_split_role_layout_compact(kind):
     if kind == "G-LFQ":
         # role_layout = 2: mixed warps through the fused gq::enqueue_or_dequeue (address-matched WAVEFAA inside a
         # converged warp, reading G10); FULL- and EMPTY-heavy histories small enough for the exact search
-        for pf, seed in ((0.25, 1), (0.75, 2), (0.5, 3)):
-            r, msg = check_tiny_split(kind, pf, seed, threads=32, ops=8, capacity=4, exact=True, role_layout=2)
-            assert "linearizable" in msg
-            check_tiny_split(kind, pf, seed, role_layout=2)
+        # role_layout = 2 is gq::enqueue_or_dequeue_step (a lane that has to wait in line hands the wait back, D12: with n = 4
+        # most operations of these runs span several calls), 4 the blocking form, 3 homogeneous warps through the step form
+        for layout in (2, 4):
+            for pf, seed in ((0.25, 1), (0.75, 2), (0.5, 3)):
+                r, msg = check_tiny_split(kind, pf, seed, threads=32, ops=8, capacity=4, exact=True, role_layout=layout)
+                assert "linearizable" in msg
+                check_tiny_split(kind, pf, seed, role_layout=layout)
+        check_tiny_split(kind, 0.5, 4, role_layout=3)
+        # BJ config 3 shape through the step form, both loop modes: counts, checksums and what is left must agree
+        n = 1 << 20
+        pre = np.arange(n // 2, dtype=np.uint32)
+        for pf, conv in ((0.5, 1), (0.25, 0), (0.9, 1)):
+            q = make(kind, n)
+            try:
+                gq.queue_prefill(q, pre)
+                r = gq.run_split(q, threads=0, producer_fraction=pf, seed=11, value_base=n // 2, role_layout=2, converged=conv,
+                                 warmup_ms=2, duration_ms=10)
+                left = gq.queue_drain(q, n + 1)
+            finally:
+                gq.queue_destroy(q)
+            conserve(r, left, pre)
     else:
         q = make(kind, 16, max_threads=64)
         try:
