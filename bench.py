@@ -409,6 +409,15 @@ def run_ours(args, rank, world, local_rank):
                         ptc[str(pf)] = {"enq_mops": round(r["succ_enq"] / r["meas_seconds"] / 1e6, 1),
                                         "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1)}
                     sweep["split_lfq_role_layout_1"] = ptc
+                    ptf = {}            # mixed warps through the resumable fused operation (role_layout = 2, D12)
+                    for pf in (0.1, 0.25, 0.5, 0.75, 0.9):
+                        gq.queue_reset(qq)
+                        gq.queue_prefill(qq, pre)
+                        r = gq.run_split(qq, threads=fk, warmup_ms=WARMUP_MS, duration_ms=DURATION_MS, producer_fraction=pf,
+                                         seed=1, value_base=1 << 19, role_layout=2, converged=CONVERGED)
+                        ptf[str(pf)] = {"enq_mops": round(r["succ_enq"] / r["meas_seconds"] / 1e6, 1),
+                                        "deq_mops": round(r["succ_deq"] / r["meas_seconds"] / 1e6, 1)}
+                    sweep["split_lfq_role_layout_2"] = ptf
                 gq.queue_destroy(qq)
                 sweep["split_" + name] = pts
             except gq.GqError as e:

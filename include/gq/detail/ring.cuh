@@ -32,6 +32,8 @@ struct RingView {
   uint32_t  prefetch;   // > 0: rings too large to stay L2-resident: pull the slot `prefetch` tickets ahead into L2
   uint32_t  id;         // 0 = AQ (or the only ring), 1 = FQ: names the ring in traces and latency probes (debug.cuh)
   uint32_t  spin_ns;    // D2: a parked dequeuer re-reads its slot without any nap for this long, then backs off
+  uint32_t  slow_nap;   // G-WFQ: longest nap of a thread that lost a SLOWFAA round, ns (<= 1024: Backoff's own ladder only)
+  uint32_t  _pad0;
   detail::BlockFunnel* fhead;   // block-level ticket funnels of the calling block (shared memory; D11), or nullptr:
   detail::BlockFunnel* ftail;   // set by the kernel on its own copy of the view (with_funnels, queue.cuh)
 };
@@ -40,13 +42,14 @@ namespace detail {
 
 enum : int { RING_OK = 0, RING_EMPTY = 1, RING_RETRY = 2, RING_PENDING = 3 };
 // A dequeue attempt that waits in line (D2) without blocking its caller: try_deq hands the wait back (RING_PENDING) with the
-// ticket it holds, and the caller comes back later with the same record; the parking budget is then counted in looks at the
-// slot, `step_ns` each.  The holder of a ticket MUST come back until the attempt ends otherwise: the enqueuer that draws the
-// same ticket will install an item for it.
+// ticket it holds, and the caller comes back later with the same record; the parking budget (park_ns) then runs in real
+// time (%globaltimer) from the first look at the vacant slot.  The holder of a ticket MUST come back until the attempt ends
+// otherwise: the enqueuer that draws the same ticket will install an item for it.
 struct DeqWait {
   uint64_t ticket = 0;
-  uint32_t waited = 0;     // ns of the parking budget used so far; 0 = no attempt pending
-  uint32_t step_ns = 2048; // what one round of the caller's loop is charged
+  uint64_t since = 0;      // %globaltimer of the first look at the vacant slot; 0 = no attempt pending
+  __device__ __forceinline__ bool pending() const { return since != 0; }
+  __device__ __forceinline__ void clear() { since = 0; }
 };
 // GQ_F_* bits of gq.h that reach the device (kept numerically identical)
 enum : uint32_t { kPerLaneFaa = 1u, kNoProbe = 2u, kNoDeqSpin = 4u, kNoOptCas = 8u, kPlainThrStore = 16u,
@@ -337,7 +340,7 @@ struct Ring {
   //     test is then made with the ticket in the place of Head, and parking (D2) is skipped when it
   //     says "empty" or Threshold was negative, which leaves the listing's own steps.  kThrFirst
   //     restores the listed order.
-  //  nb != nullptr: non-blocking parking (DeqWait above).  nb->waited != 0 resumes the attempt that holds nb->ticket.
+  //  nb != nullptr: non-blocking parking (DeqWait above).  nb->pending() resumes the attempt that holds nb->ticket.
   template <class Finalize>
   __device__ __forceinline__ static int try_deq(const RingView& r, uint32_t* x, uint64_t* h_out, const Finalize& fin,
                                                 bool probe = false, uint32_t flags = 0, DeqWait* nb = nullptr) {
@@ -345,7 +348,7 @@ struct Ring {
     int64_t thr;
     uint64_t h;
     const bool listed = probe || (flags & kThrFirst);
-    const bool resume = nb && nb->waited != 0;
+    const bool resume = nb && nb->pending();
     GQ_TIC(t0);
     if (resume) {
       h = nb->ticket;                                                  // drawn by the call that returned RING_PENDING
@@ -372,7 +375,11 @@ struct Ring {
     uint64_t* sp = slot(r, j);
     // park budget in ns: every look at the slot counts its nap plus kPollNs (an L2 round trip under load)
     constexpr uint32_t kPollNs = 384;
-    uint32_t waited = resume ? nb->waited : 0u, nap = 0;
+    uint32_t waited = 0, nap = 0;
+    if (resume) {                                                      // real time spent in line so far (never 0: 0 = first look)
+      const uint64_t dt = globaltimer_ns() - nb->since;
+      waited = dt >= 0xFFFFFFFFull ? 0xFFFFFFFFu : (dt ? (uint32_t)dt : 1u);
+    }
     GQ_TIC(t1);
     for (;;) {
       // L176.  Acquire in every build: it is the consumer side of the hand-over contract of queue.cuh (reading G15): what a
@@ -425,8 +432,7 @@ struct Ring {
           // The first spin_ns are pure re-reading (the front of the line: the hand-over is detected one nap
           // earlier), after that the nap ladder 32 ns .. park_nap keeps the many threads further back quiet.
           if (nb) {                                                    // wait handed back to the caller, ticket kept
-            nb->ticket = h;
-            nb->waited = waited + nb->step_ns;
+            if (!resume) { nb->ticket = h; nb->since = globaltimer_ns(); }
             return RING_PENDING;
           }
           if (waited >= r.spin_ns && r.park_nap) { nap = nap ? (nap * 2 < r.park_nap ? nap * 2 : r.park_nap) : 32; __nanosleep(nap); }

@@ -172,6 +172,24 @@ __device__ __forceinline__ int dequeue(const LfqView& q, thread_ctx& ctx, uint32
 }
 
 
+namespace detail {
+// Per-lane choice between the two rings of ONE queue.  Only the fields that differ between AQ and FQ are selected (entries,
+// hot words, id, funnels); sizes, the Threshold reset value and the parking constants are the same for both rings (one N, one
+// gq_opts) and stay warp-uniform kernel parameters.  (Selecting whole RingViews per lane cost the fused operations a 48-byte
+// stack frame: 1.1 sectors of local-memory stores per operation in the ncu capture.)
+__device__ __forceinline__ RingView pick_ring(bool first, const RingView& a, const RingView& b) {
+  RingView r = a;
+  r.entry = first ? a.entry : b.entry;
+  r.head = first ? a.head : b.head;
+  r.tail = first ? a.tail : b.tail;
+  r.threshold = first ? a.threshold : b.threshold;
+  r.id = first ? a.id : b.id;
+  r.fhead = first ? a.fhead : b.fhead;
+  r.ftail = first ? a.ftail : b.ftail;
+  return r;
+}
+}  // namespace detail
+
 // Fused operation for warps whose lanes have different roles (BASELINE.json config 3: the role of every
 // thread is drawn from the seed, so every warp is a mix of producers and consumers).  Called as two
 // separate operations the two groups of a warp run one after the other (SIMT divergence) and their
@@ -189,7 +207,7 @@ __device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& 
   using R = Ring<LfqFmt, false, kWarpFaa>;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   if (q.flags & kFencedPayload) return is_enq ? enqueue<false, kWarpFaa>(q, ctx, *v, retries) : dequeue<false, kWarpFaa>(q, ctx, v, retries);
-  RingView r1 = is_enq ? q.fq : q.aq, r2 = is_enq ? q.aq : q.fq;        // per-lane ring pair
+  const RingView r1 = pick_ring(is_enq, q.fq, q.aq), r2 = pick_ring(is_enq, q.aq, q.fq);   // per-lane ring pair
   const uint32_t hbit = is_enq ? 2u : 1u;
   uint32_t idx;
   uint64_t h1 = 0;
@@ -227,7 +245,7 @@ __device__ __forceinline__ int enqueue_or_dequeue(const LfqView& q, thread_ctx& 
 // converged chain of L2 round trips per call whatever the number of lanes that wait.
 // Contract: after PENDING the thread must call again with the same `st`, role and *v until it gets another result (it holds
 // a ticket; the enqueuer of that ticket will install an entry for it).  The operation's interval in a history runs from
-// its first call to the call that completes it.  The parking budget (gq_opts.park_ns) is charged st.step_ns per call.
+// its first call to the call that completes it.  The parking budget (gq_opts.park_ns) runs in real time from the first call.
 using op_state = detail::DeqWait;
 enum : int { PENDING = 3 };
 template <int kWarpFaa = true>
@@ -237,7 +255,7 @@ __device__ __forceinline__ int enqueue_or_dequeue_step(const LfqView& q, thread_
   using R = Ring<LfqFmt, false, kWarpFaa>;
   uint64_t dummy = 0; if (!retries) retries = &dummy;
   if (q.flags & kFencedPayload) return is_enq ? enqueue<false, kWarpFaa>(q, ctx, *v, retries) : dequeue<false, kWarpFaa>(q, ctx, v, retries);
-  RingView r1 = is_enq ? q.fq : q.aq, r2 = is_enq ? q.aq : q.fq;        // per-lane ring pair
+  const RingView r1 = pick_ring(is_enq, q.fq, q.aq), r2 = pick_ring(is_enq, q.aq, q.fq);   // per-lane ring pair
   const uint32_t hbit = is_enq ? 2u : 1u;
   uint32_t idx = 0;
   uint64_t h1 = 0;
@@ -251,14 +269,14 @@ __device__ __forceinline__ int enqueue_or_dequeue_step(const LfqView& q, thread_
       if (GQ_STUCK(sn, 6, ctx.tid, r1.head, r1.tail)) { s = RING_EMPTY; break; }
       s = R::try_deq(r1, &idx, &h1, NoFinalize{}, probe, q.flags, &st);
       if (s != RING_RETRY) break;
-      st.waited = 0;                                                   // that ticket is spent: next attempt draws a new one
+      st.clear();                                                      // that ticket is spent: next attempt draws a new one
       ++*retries;
       probe = true;
       bo.pause();
     }
   }
   if (s == RING_PENDING) { GQ_TOC(is_enq ? LAT_STEP_PENDING_ENQ : LAT_STEP_PENDING_DEQ, t_op, h1); return PENDING; }
-  st.waited = 0;
+  st.clear();
   if (s == RING_EMPTY) {
     ctx.hungry |= hbit;
     return is_enq ? FULL : EMPTY;

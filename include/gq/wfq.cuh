@@ -108,6 +108,7 @@ struct Wf {
     WfqRecord* mine = rec(r, me);
     uint64_t c = 0;
     Backoff bo;
+    uint32_t lost_nap = 512;
     [[maybe_unused]] uint32_t sn1 = 0, sn2 = 0;
     for (;;) {
       if (GQ_STUCK(sn1, (kDeq ? 11 : 10) | r.id << 8, me, G, L, kDeq ? r.tail : r.head, r.threshold)) return false;
@@ -142,6 +143,10 @@ struct Wf {
       const uint64_t g0 = (c << S) | kNull;
       if (cas_acq_rel(G, g0, ((c + 1) << S) | me) == g0) break;        // L262: <c,NULL> -> <c+1,tid>; release: the record is visible to whoever reads this ThrIdx
       bo.pause();                                                      // lost the round: thousands of losers must not keep G busy
+      // Backoff's ladder ends at 1 us; k losers that come back every microsecond ask G's L2 line for k atomics per microsecond,
+      // it serves 1.5 per ns (C1), and the round's winner, whose two dependent CAS on G ARE the round, waits in that line too.
+      // RingView::slow_nap (about 1 ns per launched thread) lets the ladder go on.  Still a bounded delay per lost round.
+      if (bo.ns >= 1024 && r.slow_nap > 1024) { lost_nap = lost_nap * 2 < r.slow_nap ? lost_nap * 2 : r.slow_nap; if (lost_nap > 1024) __nanosleep(lost_nap - 1024); }
     }
     ++(kDeq ? mine->n_head_inc : mine->n_tail_inc);
     if (kDeq) faa_relaxed(reinterpret_cast<uint64_t*>(r.threshold), (uint64_t)-1ll);   // L264-266

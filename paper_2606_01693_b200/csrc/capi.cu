@@ -473,7 +473,10 @@ static int dispatch(gq_queue* q, Fn&& fn) {
 }
 static void set_nthreads(LfqView&, uint32_t) {}
 static void set_nthreads(DlfqView&, uint32_t) {}
-static void set_nthreads(WfqView& v, uint32_t n) { v.nthreads = n; }
+static void set_nthreads(WfqView& v, uint32_t n) {
+  v.nthreads = n;
+  v.aq.slow_nap = v.fq.slow_nap = std::min(std::max(n, 1024u), 65536u);   // about 1 ns per thread that can lose a SLOWFAA round
+}
 static void set_nthreads(YmcView& v, uint32_t n) { v.nthreads = n; }
 
 // slow-path statistics live in the per-thread records; sum and clear them after a run

@@ -154,10 +154,13 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
       op_state st;
       uint32_t iter = 0;
       uint64_t t_call = 0;
+      // a thread has one role: one set of tallies in the loop (the kernel sits at its register limit), sorted by role afterwards
+      uint32_t n_succ = 0, n_fail = 0, n_tot = 0, n_tot_fail = 0;
+      uint64_t sum = 0;
       for (;;) {
         uint32_t v = payload_of(p, ltid, iter);
         const uint32_t v_in = v;
-        if (kHist && st.waited == 0) {
+        if (kHist && !st.pending()) {
           if (p.jitter_ns) __nanosleep(mix32(p.seed ^ (ltid * 0x85ebca6bu) ^ (iter * 2u + 0x1234567u)) % (p.jitter_ns + 1));
           t_call = globaltimer_ns();
         }
@@ -170,13 +173,14 @@ __global__ void __launch_bounds__(512, 2) bench_kernel(Q q, BenchParams p, uint6
           if (kHist) *my++ = do_enq ? gq_hist_rec{ltid, GQ_OP_ENQ, v_in, (uint32_t)s, 0u, 0u, t_call, now}
                                     : gq_hist_rec{ltid, GQ_OP_DEQ, 0u, (uint32_t)s, s == OK ? v : 0u, 0u, t_call, now};
           const bool in = now >= tw && now < te;
-          if (do_enq) { if (s == OK) { ++a.tot_enq; a.sum_enq += v_in; a.succ_enq += in; } else { ++a.tot_full; a.full += in; } }
-          else        { if (s == OK) { ++a.tot_deq; a.sum_deq += v; a.succ_deq += in; } else { ++a.tot_empty; a.empty += in; } }
+          if (s == OK) { ++n_tot; sum += v; n_succ += in; } else { ++n_tot_fail; n_fail += in; }   // v: the payload put in / taken out
           ++iter;
           done = fixed ? (iter >= p.ops_per_thread) : (now >= te);   // a pending operation is always brought to its end
         }
         if (loop_done(p, act, done)) break;
       }
+      if (do_enq) { a.succ_enq = n_succ; a.full = n_fail; a.tot_enq = n_tot; a.tot_full = n_tot_fail; a.sum_enq = sum; }
+      else        { a.succ_deq = n_succ; a.empty = n_fail; a.tot_deq = n_tot; a.tot_empty = n_tot_fail; a.sum_deq = sum; }
     } else if (!split) {
       uint32_t act = __activemask();
       for (uint32_t iter = 0;; ++iter) {
